@@ -1,0 +1,75 @@
+"""Oracle (test infrastructure): the low-lying modes of Q^2, section 2.3 (L77-93).
+
+"The spectrum of Q in the vicinity of the origin can be reliably determined by minimizing the Ritz
+functional of Q^2" - what is determined is the set of the l lowest eigenpairs of Q^2.
+The oracle therefore takes the plain definition: a dense Hermitian eigendecomposition where that is
+possible (4^4), a library Lanczos (`scipy.sparse.linalg.eigsh`) on the oracle's own Q^2 otherwise.
+Eigenvectors are unique only up to rotations inside (near-)degenerate clusters, so tests compare
+eigenvalues, residues and projector actions, never raw vectors (reading R10).
+"""
+import numpy as np
+
+
+def lowest_modes_dense(Qmat, l):
+    """l lowest eigenpairs of Q^2 from the dense matrix of Q: Q = W Lambda W^dagger => Q^2 has the same
+    eigenvectors with eigenvalues Lambda^2.  Returns (theta[l] ascending, V[N, l])."""
+    lam, W = np.linalg.eigh(Qmat)
+    order = np.argsort(lam * lam)[:l]
+    return (lam[order] ** 2), W[:, order]
+
+
+def lowest_modes_eigsh(Q, shape, l, tol=1e-10, ncv=None, seed=7, maxiter=None):
+    """l lowest eigenpairs of Q^2 by library Lanczos on the callable Q (shape = field shape)."""
+    from scipy.sparse.linalg import LinearOperator, eigsh
+
+    n = int(np.prod(shape))
+    count = [0]
+
+    def mv(x):
+        count[0] += 2
+        return Q(Q(x.reshape(shape))).reshape(n)
+
+    op = LinearOperator((n, n), matvec=mv, dtype=np.complex128)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    v0 = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    theta, vec = eigsh(op, k=l, which="SA", tol=tol, ncv=ncv, v0=v0, maxiter=maxiter)
+    order = np.argsort(theta)
+    return theta[order], [vec[:, i].reshape(shape) for i in order], count[0]
+
+
+def orthonormalise(V):
+    """Modified Gram-Schmidt (twice) on a list of vectors."""
+    out = []
+    for v in V:
+        w = v.copy()
+        for _ in range(2):
+            for u in out:
+                w = w - np.vdot(u.reshape(-1), w.reshape(-1)) * u
+        out.append(w / np.linalg.norm(w.reshape(-1)))
+    return out
+
+
+def approximate_low_space(Q, shape, l, qnorm, cut, degree=24, sweeps=3, seed=11):
+    """A cheap, APPROXIMATE low-mode space of Q^2 for the large lattices where a converged CPU
+    eigen-solve takes too long: `sweeps` rounds of a degree-`degree` Chebyshev filter in Q^2 that damps
+    the interval [cut, qnorm^2], each followed by orthonormalisation.  The result is an orthonormal set
+    V that is only roughly invariant under Q; eq. 2.11 is well defined for ANY orthonormal V (its
+    Rayleigh-Ritz pairs (nu_k, u_k) are then inputs shared by oracle and CUDA path), so this is an
+    input-preparation step for the D_N parity test at 16^3x32, not a statement about eigenvectors."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    V = [rng.standard_normal(shape) + 1j * rng.standard_normal(shape) for _ in range(l)]
+    V = orthonormalise(V)
+    a, b = cut, qnorm * qnorm
+    e, c0 = (b - a) / 2.0, (b + a) / 2.0
+
+    def filt(v):
+        # T_degree((Q^2 - c0)/e) v by the three-term recurrence
+        t0 = v
+        t1 = (Q(Q(v)) - c0 * v) / e
+        for _ in range(degree - 1):
+            t0, t1 = t1, 2.0 * (Q(Q(t1)) - c0 * t1) / e - t0
+        return t1
+
+    for _ in range(sweeps):
+        V = orthonormalise([filt(v) for v in V])
+    return V
