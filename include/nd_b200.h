@@ -1,0 +1,164 @@
+/* nd_b200.h - C-ABI boundary of the B200-native Wilson-Dirac / Neuberger-Dirac hot path of
+ * arXiv:1010.5636 ("Implementation of the Neuberger-Dirac operator on GPUs", PAPER.md).
+ *
+ * Every step behind these calls runs in hand-written CUDA kernels for sm_100a (csrc/ of the package).
+ * There is no CPU fallback: without a CUDA device nd_create() fails with ND_ERR_CUDA.
+ *
+ * Conventions
+ * -----------
+ *  - Opaque context; EVERY call returns an int status (ND_OK = 0, negative = error).  No exceptions, no
+ *    global state.  nd_last_error(ctx) gives a human-readable message owned by the context.
+ *  - Field memory is CALLER-OWNED DEVICE memory (e.g. torch tensors' data_ptr()).  A device spinor occupies
+ *    nd_spinor_bytes(ctx) bytes and must be 16-byte aligned.  The context owns only: the compressed gauge
+ *    field, reduction scratch, polynomial coefficients, a *pointer* to the caller's low-mode block.
+ *  - Work is enqueued on the cudaStream_t given to nd_create (0 = legacy default stream).  Calls that return
+ *    host scalars synchronise that stream; everything else is asynchronous.
+ *  - "host AoS" = canonical site-major arrays, x3 fastest:
+ *        spinor  psi[x0][x1][x2][x3][spin 4][colour 3]           complex (re, im interleaved)
+ *        links   U[mu 4][x0][x1][x2][x3][row 3][col 3]           complex
+ *    dims = (L0, L1, L2, L3) with L0 the time extent T (mu = 0 is time).
+ *  - "device SoA" = the library's own layout: planes of 128-bit words,
+ *        fp32: 6 planes of float4 [V]   (plane p = reals 4p..4p+3 of the 24 reals spin-major)
+ *        fp64: 12 planes of double2 [V] (plane p = complex component p = spin*3 + colour)
+ *    site index = ((x0*L1 + x1)*L2 + x2)*L3 + x3.  Convert with nd_pack_spinor / nd_unpack_spinor.
+ *  - Complex scalars cross the boundary as double[2] = (re, im).  All reductions accumulate in fp64 in both
+ *    precisions.
+ *  - Stencil calls require out != in (and != tmp); violating it returns ND_ERR_BAD_ARG.
+ */
+#ifndef ND_B200_H
+#define ND_B200_H
+
+#include <stddef.h>
+
+#if defined(__GNUC__)
+#define ND_API __attribute__((visibility("default")))
+#else
+#define ND_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nd_ctx nd_ctx;
+
+enum {
+    ND_OK = 0,
+    ND_ERR_BAD_ARG = -1,         /* null pointer, bad enum value, aliasing, size mismatch */
+    ND_ERR_BAD_STATE = -2,       /* gauge field / polynomial / low modes not set yet */
+    ND_ERR_NOT_SU3 = -3,         /* nd_set_gauge: a link violates U^dagger U = 1, det U = 1 beyond tolerance */
+    ND_ERR_RECON8_SINGULAR = -4, /* nd_set_gauge with recon 8: |a2|^2+|a3|^2 below threshold (e.g. unit links) */
+    ND_ERR_CUDA = -5,            /* CUDA runtime error (message in nd_last_error) */
+    ND_ERR_NO_CONVERGENCE = -6,  /* nd_lowmodes_compute: maxit reached before tol */
+    ND_ERR_NOMEM = -7
+};
+
+/* ---------------------------------------------------------------------------------------------- lifecycle
+ * Geometry of the 4D lattice of eq. 2.1 and the storage choices of section 2.1
+ * (PAPER.md:L44-50).
+ *   dims     [in, host]  (L0=T, L1, L2, L3), each >= 2
+ *   prec     32 or 64: arithmetic and storage type of spinors and links
+ *   recon    18, 12 or 8: real parameters stored per SU(3) link (12: eq. 2.3; 8: PAPER.md:L46, R8)
+ *   bc_time  +1 periodic / -1 antiperiodic in mu = 0 (space is periodic)
+ *   device   CUDA device ordinal
+ *   stream   cudaStream_t as void* (may be NULL)
+ * On failure *ctx is NULL.  nd_destroy frees everything the context owns. */
+ND_API int nd_create(nd_ctx** ctx, const int dims[4], int prec, int recon, int bc_time, int device, void* stream);
+ND_API int nd_destroy(nd_ctx* ctx);
+ND_API const char* nd_last_error(const nd_ctx* ctx);   /* never NULL; valid until the next call on ctx */
+ND_API int nd_set_stream(nd_ctx* ctx, void* stream);
+ND_API long long nd_volume(const nd_ctx* ctx);          /* number of sites V */
+ND_API size_t nd_spinor_bytes(const nd_ctx* ctx);       /* bytes of one device SoA spinor = 24 * V * prec/8 */
+ND_API size_t nd_gauge_bytes(const nd_ctx* ctx);        /* bytes of the compressed device gauge field */
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
+ND_API long long nd_launch_count(const nd_ctx* ctx);
+
+/* ------------------------------------------------------------------------------------------------- gauge
+ * nd_set_gauge: take the canonical AoS links (src_prec 32: complex64, 64: complex128; on_device != 0: the
+ * pointer is device memory, else host memory), check them (ND_ERR_NOT_SU3 / ND_ERR_RECON8_SINGULAR),
+ * compress to `recon` reals and reorder to the device layout.  The input is not kept.
+ * nd_get_gauge: reconstruct the full 3x3 links from the stored parameters into a canonical complex128 AoS
+ * array (round-trip pin of eq. 2.3). */
+ND_API int nd_set_gauge(nd_ctx* ctx, const void* links_aos, int src_prec, int on_device);
+ND_API int nd_get_gauge(nd_ctx* ctx, void* links_aos_c128, int on_device);
+/* Diagnostics of the last nd_set_gauge: out[0] = max |U^dagger U - 1| entry, out[1] = max |det U - 1|,
+ * out[2] = min over links of N = |a2|^2 + |a3|^2 (conditioning of the 8-parameter form). */
+ND_API int nd_gauge_stats(nd_ctx* ctx, double out[3]);
+
+/* ------------------------------------------------------------------------------------------------ layout
+ * Canonical AoS (prec 32: complex64 / 64: complex128; host or device) <-> device SoA in the context's
+ * precision.  `soa` is always device memory of nd_spinor_bytes(ctx). */
+ND_API int nd_pack_spinor(nd_ctx* ctx, const void* aos, int aos_prec, int aos_on_device, void* soa);
+ND_API int nd_unpack_spinor(nd_ctx* ctx, const void* soa, void* aos, int aos_prec, int aos_on_device);
+
+/* --------------------------------------------------------------------------------------------- operators
+ * out = Q in,  Q = gamma5 D_W,
+ *   D_W phi(x) = (4+m) phi(x) - 1/2 sum_{mu=0..3} [ U_mu(x)(1-gamma_mu) phi(x+mu^)
+ *                                                 + U_mu(x-mu^)^dagger (1+gamma_mu) phi(x-mu^) ]
+ * (eq. 2.1-2.2; chiral gamma basis, R2).  out, in: device SoA spinors.
+ * nd_apply_Q2: out = Q (Q in) through the caller's temporary tmp. */
+ND_API int nd_apply_Q(nd_ctx* ctx, void* out, const void* in, double m);
+ND_API int nd_apply_Q2(nd_ctx* ctx, void* out, const void* in, void* tmp, double m);
+/* out = s0 * Q(in) + s1*v1 + s2*v2 + s3*v3 with real scalars: the stencil with the vector recurrence folded
+ * into its epilogue (the fused Clenshaw step of PAPER.md:L66).  v_i may be NULL when s_i == 0; out may
+ * alias any v_i but not in. */
+ND_API int nd_apply_Q_axpbycz(nd_ctx* ctx, void* out, const void* in, double m, double s0,
+                       double s1, const void* v1, double s2, const void* v2, double s3, const void* v3);
+
+/* ----------------------------------------------------------------------------- sign function / D_N set-up
+ * nd_cheb_coeffs (host utility, no GPU): coefficients c[0..n] of P_n(y) = sum_k c_k T_k((2y-1-eps)/(1-eps))
+ * approximating y^{-1/2} on [eps, 1] (eq. 2.5-2.6; Chebyshev interpolation, full c_0) and the
+ * measured delta = max_{eps<=y<=1} |1 - sqrt(y) P(y)| (eq. 2.6). */
+ND_API int nd_cheb_coeffs(int n, double eps, double* c, double* delta);
+/* Polynomial used by nd_apply_sign / nd_apply_DN: degree n, coefficients c[0..n] (host, copied), eps, the
+ * norm bound qnorm >= ||Q|| (X = Q/qnorm) and the kernel mass m (= -(1+s), eq. 2.4). */
+ND_API int nd_set_sign_poly(nd_ctx* ctx, int n, const double* c, double eps, double qnorm, double m);
+/* Low-mode set of eq. 2.7: l orthonormal approximate eigenvectors u_k of Q (device SoA,
+ * contiguous: vector k at byte offset k*nd_spinor_bytes) with Ritz values nu[k] (host).  The pointer is kept,
+ * not copied; l = 0 clears it. */
+ND_API int nd_set_lowmodes(nd_ctx* ctx, int l, const void* u_soa, const double* nu);
+
+/* ------------------------------------------------------------------------------------------- sign / D_N
+ * nd_apply_sign: out = sum_k sign(nu_k) u_k <u_k,in> + (1 - sum_k u_k u_k^dagger) X P_n(X^2) in   (eq. 2.11,
+ * PAPER.md:L112; without low modes: eq. 2.5).  P_n(X^2) by the Clenshaw recurrence with each
+ * step's vector update fused into the second stencil of Q^2: 2n+1 stencil launches.
+ * nd_apply_DN: out = prefactor * (in + gamma5 sign(Q) in)   (eq. 2.4).
+ * work = 3 caller-owned device spinors, contiguous (3*nd_spinor_bytes).  use_graph != 0 replays the launch
+ * sequence as a CUDA graph cached on (out, in, work). */
+ND_API int nd_apply_sign(nd_ctx* ctx, void* out, const void* in, void* work, int use_graph);
+ND_API int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor, void* work, int use_graph);
+
+/* --------------------------------------------------------------------------------------------- low modes
+ * The l lowest eigenpairs of Q^2 followed by the Rayleigh-Ritz step of Q in their span
+ * (PAPER.md:L81): on return u_out holds u_k (device SoA, l vectors), nu[k] the Ritz values of Q (ascending in
+ * nu^2), resid[k] = ||(Q - nu_k) u_k|| (eq. 2.8).  `m` is the kernel mass.  work: (2*(l+lextra)+4) device spinors.
+ * Method: Chebyshev-filtered subspace iteration on Q^2 + Rayleigh-Ritz (R13); stops when all l
+ * residuals of Q^2 are <= tol or after maxit outer iterations (ND_ERR_NO_CONVERGENCE, results still filled).
+ * stats (may be NULL): [0] outer iterations, [1] stencil applications. */
+ND_API int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, double m, double tol, int maxit,
+                        unsigned long long seed, void* u_out, double* nu, double* resid, void* work,
+                        long long* stats);
+
+/* ------------------------------------------------------------------------------------------------ BLAS-1
+ * Spinor-field vector operations (device SoA).  a = (re, im).
+ *   nd_axpy:       y <- a x + y            nd_scale: x <- a x         nd_copy: y <- x
+ *   nd_dot:        out = <x, y> = sum conj(x) y      (host result; synchronises)
+ *   nd_norm2:      out = <x, x>
+ *   nd_gamma5:     y <- gamma5 x  (y may alias x)
+ *   nd_block_dot:  out[2k..2k+1] = <v_k, x>, k < l   (one pass over x and the block; host result)
+ *   nd_block_axpy: y <- y + sum_k a[k] v_k           (a = l complex numbers on the host)
+ *   nd_gaussian:   fill x with Re, Im ~ N(0,1) from a counter-based generator (Philox-4x32-10 + Box-Muller) */
+ND_API int nd_axpy(nd_ctx* ctx, const double a[2], const void* x, void* y);
+ND_API int nd_scale(nd_ctx* ctx, const double a[2], void* x);
+ND_API int nd_copy(nd_ctx* ctx, void* y, const void* x);
+ND_API int nd_dot(nd_ctx* ctx, const void* x, const void* y, double out[2]);
+ND_API int nd_norm2(nd_ctx* ctx, const void* x, double* out);
+ND_API int nd_gamma5(nd_ctx* ctx, void* y, const void* x);
+ND_API int nd_block_dot(nd_ctx* ctx, int l, const void* v, const void* x, double* out2l);
+ND_API int nd_block_axpy(nd_ctx* ctx, int l, const double* a2l, const void* v, void* y);
+ND_API int nd_gaussian(nd_ctx* ctx, void* x, unsigned long long seed);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ND_B200_H */

@@ -1,0 +1,154 @@
+// nd_internal.cuh - shared declarations of the CUDA path (context, device layout traits, complex helpers).
+// Product code: nothing here is shared with oracle/.
+//
+// Device layout ("the data layout ... coalescing"):
+//   site index s = ((x0*L1 + x1)*L2 + x2)*L3 + x3  (x3 fastest, the warp runs along x3)
+//   spinor : NV planes of 128-bit words, word (p, s) at  f[p*V + s]
+//            fp32: NV = 6,  float4  = reals 4p..4p+3 of the 24 reals (spin-major, colour, re/im)
+//            fp64: NV = 12, double2 = complex component p = spin*3 + colour
+//   links  : word (mu, p, s) at g[(mu*NL + p)*V + s]; the P = recon reals of a link in NL words of LVec
+//            P=18: rows a,b,c (9 complex); P=12: rows a,b (eq. 2.3 on rows); P=8: a2,a3,b1,theta1,theta2
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/nd_b200.h"
+
+struct nd_graph_entry {
+    void* out;
+    const void* in;
+    void* work;
+    int kind;            // 0 sign, 1 D_N
+    double prefactor;
+    cudaGraphExec_t exec;
+    long long nodes;     // kernel launches one replay stands for
+};
+
+struct nd_ctx {
+    int dims[4];
+    long long V;
+    int prec, recon, bc;
+    int device;
+    cudaStream_t stream;
+    void* gauge;
+    size_t gauge_bytes;
+    bool gauge_set;
+    double gstats[3];
+    // reductions
+    double* d_partial;   // [ND_MAX_RED_BLOCKS * 2 * ND_MAX_BLOCK_L]
+    double* d_result;    // [2 * ND_MAX_BLOCK_L * 2]
+    double* h_result;    // pinned, same size
+    double* d_coef;      // [2 * ND_MAX_BLOCK_L] device copy of block-axpy coefficients
+    double* d_nu;        // [ND_MAX_BLOCK_L] Ritz values on the device (sign of nu_k)
+    // sign polynomial
+    std::vector<double> cheb;
+    int n;
+    double eps, qnorm, m_sign;
+    bool poly_set;
+    // low modes
+    int l;
+    const void* u;
+    std::vector<double> nu;
+    std::vector<nd_graph_entry> graphs;
+    long long launches;
+    bool capturing;
+    char err[512];
+};
+
+constexpr int ND_MAX_BLOCK_L = 256;     // max vectors in a block dot / block axpy
+constexpr int ND_MAX_RED_BLOCKS = 1184; // 8 x 148
+
+int nd_fail(nd_ctx* ctx, int code, const char* fmt, ...);
+int nd_cuda_check(nd_ctx* ctx, cudaError_t e, const char* what);
+#define ND_CUDA(ctx, call)                                         \
+    do {                                                           \
+        int _rc = nd_cuda_check((ctx), (call), #call);             \
+        if (_rc != ND_OK) return _rc;                              \
+    } while (0)
+#define ND_LAUNCHED(ctx)                                           \
+    do {                                                           \
+        (ctx)->launches++;                                         \
+        int _rc = nd_cuda_check((ctx), cudaGetLastError(), "launch"); \
+        if (_rc != ND_OK) return _rc;                              \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------- layout traits
+template <typename T> struct Prec;
+template <> struct Prec<float> {
+    using Vec = float4;
+    static constexpr int NV = 6;
+};
+template <> struct Prec<double> {
+    using Vec = double2;
+    static constexpr int NV = 12;
+};
+
+template <typename T, int RECON> struct LinkLayout;
+template <> struct LinkLayout<float, 18> { using LVec = float2;  static constexpr int NL = 9; };
+template <> struct LinkLayout<float, 12> { using LVec = float4;  static constexpr int NL = 3; };
+template <> struct LinkLayout<float, 8>  { using LVec = float4;  static constexpr int NL = 2; };
+template <> struct LinkLayout<double, 18> { using LVec = double2; static constexpr int NL = 9; };
+template <> struct LinkLayout<double, 12> { using LVec = double2; static constexpr int NL = 6; };
+template <> struct LinkLayout<double, 8>  { using LVec = double2; static constexpr int NL = 4; };
+
+// ---------------------------------------------------------------------------------------------- complex
+template <typename T> struct cx {
+    T re, im;
+};
+template <typename T> __host__ __device__ __forceinline__ cx<T> mk(T re, T im) { return cx<T>{re, im}; }
+template <typename T> __host__ __device__ __forceinline__ cx<T> operator+(cx<T> a, cx<T> b) { return {a.re + b.re, a.im + b.im}; }
+template <typename T> __host__ __device__ __forceinline__ cx<T> operator-(cx<T> a, cx<T> b) { return {a.re - b.re, a.im - b.im}; }
+template <typename T> __host__ __device__ __forceinline__ cx<T> operator*(cx<T> a, cx<T> b) {
+    return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re};
+}
+template <typename T> __host__ __device__ __forceinline__ cx<T> cj(cx<T> a) { return {a.re, -a.im}; }
+template <typename T> __host__ __device__ __forceinline__ cx<T> times_i(cx<T> a) { return {-a.im, a.re}; }
+template <typename T> __host__ __device__ __forceinline__ cx<T> times_mi(cx<T> a) { return {a.im, -a.re}; }
+// acc += a * b
+template <typename T> __host__ __device__ __forceinline__ void cfma(cx<T>& acc, cx<T> a, cx<T> b) {
+    acc.re = fma(a.re, b.re, acc.re);
+    acc.re = fma(-a.im, b.im, acc.re);
+    acc.im = fma(a.re, b.im, acc.im);
+    acc.im = fma(a.im, b.re, acc.im);
+}
+// acc += conj(a) * b
+template <typename T> __host__ __device__ __forceinline__ void cfma_cj(cx<T>& acc, cx<T> a, cx<T> b) {
+    acc.re = fma(a.re, b.re, acc.re);
+    acc.re = fma(a.im, b.im, acc.re);
+    acc.im = fma(a.re, b.im, acc.im);
+    acc.im = fma(-a.im, b.re, acc.im);
+}
+
+// 12 complex components of a spinor <-> the 128-bit words of its planes
+__device__ __forceinline__ void words_to_cx(const float4 (&w)[6], cx<float> (&c)[12]) {
+#pragma unroll
+    for (int p = 0; p < 6; p++) {
+        c[2 * p] = {w[p].x, w[p].y};
+        c[2 * p + 1] = {w[p].z, w[p].w};
+    }
+}
+__device__ __forceinline__ void words_to_cx(const double2 (&w)[12], cx<double> (&c)[12]) {
+#pragma unroll
+    for (int p = 0; p < 12; p++) c[p] = {w[p].x, w[p].y};
+}
+__device__ __forceinline__ void cx_to_words(const cx<float> (&c)[12], float4 (&w)[6]) {
+#pragma unroll
+    for (int p = 0; p < 6; p++) w[p] = make_float4(c[2 * p].re, c[2 * p].im, c[2 * p + 1].re, c[2 * p + 1].im);
+}
+__device__ __forceinline__ void cx_to_words(const cx<double> (&c)[12], double2 (&w)[12]) {
+#pragma unroll
+    for (int p = 0; p < 12; p++) w[p] = make_double2(c[p].re, c[p].im);
+}
+
+// ---------------------------------------------------------------------------- internal entry points (per TU)
+int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
+                double s2, const void* v2, double s3, const void* v3);
+int ndi_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out);   // d_out: 2l doubles (device)
+int ndi_block_dot2_dev(nd_ctx* ctx, int l, const void* v, const void* x0, const void* x1, double* d_out);  // 4l doubles
+int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pref);
+int ndi_read_result(nd_ctx* ctx, const double* d_src, double* h_dst, int n);              // sync copy to host
+int ndi_drop_graphs(nd_ctx* ctx);
+constexpr int ND_RESULT_DOUBLES = 4 * ND_MAX_BLOCK_L;

@@ -1,0 +1,213 @@
+// sign.cu - Chebyshev approximation of sign(Q) by a fused Clenshaw recurrence, the projected sign function and the
+// Neuberger-Dirac operator (section 2.2-2.3: eq. 2.4-2.6, 2.7, 2.11; L56-73, L81-84, L110-113).
+//
+//   sign(Q) ~ X P_n(X^2),  X = Q/qnorm,  P_n(y) = sum_{k=0}^n c_k T_k(z),  z = (2y-1-eps)/(1-eps)      (2.5; R7)
+//   Z = alpha Q^2 + beta,  alpha = 2/((1-eps) qnorm^2),  beta = -(1+eps)/(1-eps)
+//   b_n = c_n eta;  b_k = c_k eta + 2 Z b_{k+1} - b_{k+2}  (k = n-1..1);  P eta = c_0 eta + Z b_1 - b_2    (R9)
+//   chi = Q P eta / qnorm;   sign eta ~ sum_k sign(nu_k) u_k <u_k,eta> + chi - sum_k u_k <u_k,chi>           (2.11)
+//   D_N eta = prefactor (eta + gamma5 sign eta)                                                             (2.4)
+//
+// Every Clenshaw step is two stencil launches; the vector update is the epilogue of the second one
+// (nd_apply_Q_axpbycz), so the recurrence vectors are read/written exactly once per step: 2n+1 stencil launches per
+// sign application, no separate axpy kernels.  No host synchronisation anywhere: the projection coefficients stay on
+// the device, so the whole application can be replayed as one CUDA graph.
+#include <cmath>
+
+#include "nd_internal.cuh"
+
+namespace {
+
+template <typename T>
+__global__ void scale_copy_kernel(typename Prec<T>::Vec* __restrict__ y, const typename Prec<T>::Vec* __restrict__ x, T a, long long nwords) {
+    for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < nwords; w += (long long)gridDim.x * blockDim.x) {
+        typename Prec<T>::Vec v = x[w];
+        T* pv = reinterpret_cast<T*>(&v);
+#pragma unroll
+        for (int k = 0; k < (int)(sizeof(v) / sizeof(T)); k++) pv[k] *= a;
+        y[w] = v;
+    }
+}
+
+// coef_k = sign(nu_k) <u_k,eta> - <u_k,chi>   (dots = [<u,eta> (2l) | <u,chi> (2l)])
+__global__ void lowmode_coef_kernel(double* __restrict__ coef, const double* __restrict__ dots, const double* __restrict__ nu, int l) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= l) return;
+    const double sg = (nu[k] > 0.0) ? 1.0 : ((nu[k] < 0.0) ? -1.0 : 0.0);
+    coef[2 * k] = sg * dots[2 * k] - dots[2 * l + 2 * k];
+    coef[2 * k + 1] = sg * dots[2 * k + 1] - dots[2 * l + 2 * k + 1];
+}
+
+int scale_copy(nd_ctx* ctx, void* y, const void* x, double a) {
+    const long long nwords = ctx->V * (ctx->prec == 32 ? 6 : 12);
+    long long b = (nwords + 255) / 256;
+    if (ctx->prec == 32) scale_copy_kernel<float><<<(unsigned)b, 256, 0, ctx->stream>>>((float4*)y, (const float4*)x, (float)a, nwords);
+    else scale_copy_kernel<double><<<(unsigned)b, 256, 0, ctx->stream>>>((double2*)y, (const double2*)x, a, nwords);
+    ND_LAUNCHED(ctx);
+    return ND_OK;
+}
+
+// kind 0: out = sign(Q) in ; kind 1: out = prefactor (in + gamma5 sign(Q) in)
+int enqueue_sign(nd_ctx* ctx, void* out, const void* eta, void* work, int kind, double prefactor) {
+    const size_t sb = nd_spinor_bytes(ctx);
+    char* bA = (char*)work;
+    char* bB = bA + sb;
+    char* tmp = bB + sb;
+    const int n = ctx->n;
+    const double* c = ctx->cheb.data();
+    const double m = ctx->m_sign;
+    const double alpha = 2.0 / ((1.0 - ctx->eps) * ctx->qnorm * ctx->qnorm);
+    const double beta = -(1.0 + ctx->eps) / (1.0 - ctx->eps);
+    int rc;
+    if (n == 0) {
+        rc = ndi_apply_Q(ctx, out, eta, m, true, c[0] / ctx->qnorm, 0, nullptr, 0, nullptr, 0, nullptr);
+        if (rc != ND_OK) return rc;
+    } else {
+        rc = scale_copy(ctx, bA, eta, c[n]);   // b_n = c_n eta ; b_{n+1} = 0 is never materialised
+        if (rc != ND_OK) return rc;
+        for (int k = n - 1; k >= 0; k--) {
+            // tmp = Q b_{k+1};   b_k = f*(alpha Q tmp + beta b_{k+1}) - b_{k+2} + c_k eta,  f = 2 (k >= 1) or 1 (k = 0)
+            rc = ndi_apply_Q(ctx, tmp, bA, m, false, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+            if (rc != ND_OK) return rc;
+            const double f = (k >= 1) ? 2.0 : 1.0;
+            const double s2 = (k == n - 1) ? 0.0 : -1.0;
+            rc = ndi_apply_Q(ctx, bB, tmp, m, true, f * alpha, f * beta, bA, s2, bB, c[k], eta);
+            if (rc != ND_OK) return rc;
+            char* t = bA; bA = bB; bB = t;
+        }
+        // bA = P eta ;  chi = Q P eta / qnorm
+        rc = ndi_apply_Q(ctx, out, bA, m, true, 1.0 / ctx->qnorm, 0, nullptr, 0, nullptr, 0, nullptr);
+        if (rc != ND_OK) return rc;
+    }
+    const int l = ctx->l;
+    if (l > 0) {
+        rc = ndi_block_dot2_dev(ctx, l, ctx->u, eta, out, ctx->d_result);
+        if (rc != ND_OK) return rc;
+        lowmode_coef_kernel<<<(l + 63) / 64, 64, 0, ctx->stream>>>(ctx->d_coef, ctx->d_result, ctx->d_nu, l);
+        ND_LAUNCHED(ctx);
+    }
+    if (l > 0 || kind == 1) {
+        rc = ndi_block_axpy_dev(ctx, l, ctx->d_coef, ctx->u, out, kind, eta, prefactor);
+        if (rc != ND_OK) return rc;
+    }
+    return ND_OK;
+}
+
+int apply_sign_impl(nd_ctx* ctx, void* out, const void* in, void* work, int kind, double prefactor, int use_graph) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (!out || !in || !work || out == in) return nd_fail(ctx, ND_ERR_BAD_ARG, "apply_sign/DN: null or aliased argument");
+    if (!ctx->gauge_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_sign/DN: gauge field not set");
+    if (!ctx->poly_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_sign/DN: polynomial not set (nd_set_sign_poly)");
+    ND_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (!use_graph || ctx->stream == nullptr) return enqueue_sign(ctx, out, in, work, kind, prefactor);
+    for (auto& g : ctx->graphs)
+        if (g.out == out && g.in == in && g.work == work && g.kind == kind && g.prefactor == prefactor) {
+            ND_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
+            ctx->launches += g.nodes;
+            return ND_OK;
+        }
+    const long long before = ctx->launches;
+    ND_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    int rc = enqueue_sign(ctx, out, in, work, kind, prefactor);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(ctx->stream, &graph);
+    const long long nodes = ctx->launches - before;
+    ctx->launches = before;
+    if (rc != ND_OK) {
+        if (graph) cudaGraphDestroy(graph);
+        return rc;
+    }
+    ND_CUDA(ctx, e);
+    nd_graph_entry g;
+    g.out = out; g.in = in; g.work = work; g.kind = kind; g.prefactor = prefactor; g.exec = nullptr; g.nodes = nodes;
+    e = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    ND_CUDA(ctx, e);
+    if (ctx->graphs.size() >= 16) ndi_drop_graphs(ctx);
+    ctx->graphs.push_back(g);
+    ND_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
+    ctx->launches += nodes;
+    return ND_OK;
+}
+
+}  // namespace
+
+// --------------------------------------------------------------------------------------------------- C ABI
+extern "C" int nd_cheb_coeffs(int n, double eps, double* c, double* delta) {
+    if (n < 0 || !(eps > 0.0 && eps < 1.0) || !c) return ND_ERR_BAD_ARG;
+    typedef long double ld;
+    const ld pi = acosl(-1.0L);
+    std::vector<ld> f(n + 1), th(n + 1);
+    for (int j = 0; j <= n; j++) {
+        th[j] = pi * ((ld)j + 0.5L) / (ld)(n + 1);
+        const ld z = cosl(th[j]);
+        const ld y = ((1.0L - (ld)eps) * z + 1.0L + (ld)eps) / 2.0L;
+        f[j] = 1.0L / sqrtl(y);
+    }
+    for (int k = 0; k <= n; k++) {
+        ld s = 0.0L;
+        for (int j = 0; j <= n; j++) s += f[j] * cosl((ld)k * th[j]);
+        s *= 2.0L / (ld)(n + 1);
+        if (k == 0) s *= 0.5L;   // full c_0: P = sum_{k=0}^n c_k T_k as eq. 2.5 is printed
+        c[k] = (double)s;
+    }
+    if (delta) {
+        // delta = max |1 - sqrt(y) P(y)| on a geometric and a linear grid of [eps, 1] (eq. 2.6)
+        const int npts = 200001;
+        double worst = 0.0;
+        const double lr = log(1.0 / eps);
+        for (int pass = 0; pass < 2; pass++)
+            for (int i = 0; i < npts; i++) {
+                const double t = (double)i / (double)(npts - 1);
+                const double y = pass == 0 ? eps * exp(lr * t) : eps + (1.0 - eps) * t;
+                const double z = (2.0 * y - 1.0 - eps) / (1.0 - eps);
+                double b1 = 0.0, b2 = 0.0;
+                for (int k = n; k >= 1; k--) {
+                    const double b0 = c[k] + 2.0 * z * b1 - b2;
+                    b2 = b1;
+                    b1 = b0;
+                }
+                const double P = c[0] + z * b1 - b2;
+                const double d = fabs(1.0 - sqrt(y) * P);
+                if (d > worst) worst = d;
+            }
+        *delta = worst;
+    }
+    return ND_OK;
+}
+
+extern "C" int nd_set_sign_poly(nd_ctx* ctx, int n, const double* c, double eps, double qnorm, double m) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (n < 0 || !c || !(eps > 0.0 && eps < 1.0) || !(qnorm > 0.0)) return nd_fail(ctx, ND_ERR_BAD_ARG, "set_sign_poly: bad argument");
+    ctx->cheb.assign(c, c + n + 1);
+    ctx->n = n;
+    ctx->eps = eps;
+    ctx->qnorm = qnorm;
+    ctx->m_sign = m;
+    ctx->poly_set = true;
+    ndi_drop_graphs(ctx);
+    return ND_OK;
+}
+
+extern "C" int nd_set_lowmodes(nd_ctx* ctx, int l, const void* u_soa, const double* nu) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (l < 0 || l > ND_MAX_BLOCK_L || (l > 0 && (!u_soa || !nu))) return nd_fail(ctx, ND_ERR_BAD_ARG, "set_lowmodes: bad argument (0 <= l <= %d)", ND_MAX_BLOCK_L);
+    ND_CUDA(ctx, cudaSetDevice(ctx->device));
+    ndi_drop_graphs(ctx);
+    ctx->l = l;
+    ctx->u = l ? u_soa : nullptr;
+    ctx->nu.assign(nu, nu + l);
+    if (l) {
+        ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        for (int i = 0; i < l; i++) ctx->h_result[i] = nu[i];
+        ND_CUDA(ctx, cudaMemcpyAsync(ctx->d_nu, ctx->h_result, (size_t)l * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    }
+    return ND_OK;
+}
+
+extern "C" int nd_apply_sign(nd_ctx* ctx, void* out, const void* in, void* work, int use_graph) {
+    return apply_sign_impl(ctx, out, in, work, 0, 0.0, use_graph);
+}
+extern "C" int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor, void* work, int use_graph) {
+    return apply_sign_impl(ctx, out, in, work, 1, prefactor, use_graph);
+}

@@ -1,0 +1,258 @@
+// wilson.cu - the Wilson-Dirac stencil Q = gamma5 D_W (eq. 2.1-2.2) for sm_100a.
+//
+//   D_W phi(x) = (4+m) phi(x) - 1/2 sum_{mu=0..3} [ U_mu(x)(1-gamma_mu) phi(x+mu^) + U_mu(x-mu^)^dagger (1+gamma_mu) phi(x-mu^) ]
+//
+// One thread per output site, but: spin-projection to half-spinors BEFORE the SU(3) multiply,
+// links reconstructed from 12 / 8 reals in registers, 128-bit coalesced loads from the
+// plane-SoA layout, optional fused epilogue  out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3  (the Clenshaw vector
+// recurrence of PAPER.md:L66 folded into the stencil's store).
+//
+// Chiral basis (R2): gamma_mu = [[0, A_mu], [A_mu^dagger, 0]], A_0 = -1, A_k = -i sigma_k, gamma5 = diag(1,1,-1,-1).
+//   (1-gamma_mu) psi = (h, -A^dagger h),  h  = psi_up - A psi_low
+//   (1+gamma_mu) psi = (h',  A^dagger h'), h' = psi_up + A psi_low
+#include "nd_internal.cuh"
+#include "nd_su3.cuh"
+
+namespace {
+
+struct Geom {
+    int L0, L1, L2, L3;
+    long long V;
+    long long S1, S2;   // strides of x1, x0 in sites: S2 = L3 (x2 stride), S1 = L2*L3, S0 = L1*L2*L3
+    long long S0;
+    int bc;             // +1 / -1
+};
+
+template <typename T>
+__device__ __forceinline__ void load_spinor(const typename Prec<T>::Vec* __restrict__ f, long long V, long long s,
+                                            cx<T> (&c)[12]) {
+    typename Prec<T>::Vec w[Prec<T>::NV];
+#pragma unroll
+    for (int p = 0; p < Prec<T>::NV; p++) w[p] = ldg_vec(f + p * V + s);
+    words_to_cx(w, c);
+}
+
+// g = U h (colour mat-vec for both spin components of the half-spinor)
+template <typename T> __device__ __forceinline__ void mul_U(const cx<T> (&U)[3][3], const cx<T> (&h)[2][3], cx<T> (&g)[2][3]) {
+#pragma unroll
+    for (int s = 0; s < 2; s++)
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            cx<T> a = U[i][0] * h[s][0];
+            cfma(a, U[i][1], h[s][1]);
+            cfma(a, U[i][2], h[s][2]);
+            g[s][i] = a;
+        }
+}
+// g = U^dagger h
+template <typename T> __device__ __forceinline__ void mul_Udag(const cx<T> (&U)[3][3], const cx<T> (&h)[2][3], cx<T> (&g)[2][3]) {
+#pragma unroll
+    for (int s = 0; s < 2; s++)
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            cx<T> a = cj(U[0][i]) * h[s][0];
+            cfma_cj(a, U[1][i], h[s][1]);
+            cfma_cj(a, U[2][i], h[s][2]);
+            g[s][i] = a;
+        }
+}
+
+// Spin projection: h = psi_up -/+ A_mu psi_low   (SGN = -1: (1-gamma_mu), forward hop; +1: (1+gamma_mu), backward hop)
+template <typename T, int MU, int SGN>
+__device__ __forceinline__ void project(const cx<T> (&p)[12], T phase, cx<T> (&h)[2][3]) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        cx<T> u0 = p[c], u1 = p[3 + c], l0 = p[6 + c], l1 = p[9 + c];
+        cx<T> a, b;   // a = (A psi_low)_0, b = (A psi_low)_1
+        if (MU == 0) { a = {-l0.re, -l0.im}; b = {-l1.re, -l1.im}; }
+        else if (MU == 1) { a = times_mi(l1); b = times_mi(l0); }
+        else if (MU == 2) { a = {-l1.re, -l1.im}; b = l0; }
+        else { a = times_mi(l0); b = times_i(l1); }
+        cx<T> h0 = (SGN < 0) ? (u0 - a) : (u0 + a);
+        cx<T> h1 = (SGN < 0) ? (u1 - b) : (u1 + b);
+        h[0][c] = {phase * h0.re, phase * h0.im};
+        h[1][c] = {phase * h1.re, phase * h1.im};
+    }
+}
+
+// acc += (g, -/+ A^dagger g)   (SGN = -1: lower = -A^dagger g; +1: lower = +A^dagger g)
+template <typename T, int MU, int SGN>
+__device__ __forceinline__ void accumulate(const cx<T> (&g)[2][3], cx<T> (&acc)[12]) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        acc[c] = acc[c] + g[0][c];
+        acc[3 + c] = acc[3 + c] + g[1][c];
+        cx<T> d0, d1;   // A^dagger g
+        if (MU == 0) { d0 = {-g[0][c].re, -g[0][c].im}; d1 = {-g[1][c].re, -g[1][c].im}; }
+        else if (MU == 1) { d0 = times_i(g[1][c]); d1 = times_i(g[0][c]); }
+        else if (MU == 2) { d0 = g[1][c]; d1 = {-g[0][c].re, -g[0][c].im}; }
+        else { d0 = times_i(g[0][c]); d1 = times_mi(g[1][c]); }
+        if (SGN < 0) { acc[6 + c] = acc[6 + c] - d0; acc[9 + c] = acc[9 + c] - d1; }
+        else { acc[6 + c] = acc[6 + c] + d0; acc[9 + c] = acc[9 + c] + d1; }
+    }
+}
+
+template <typename T, int RECON, int MU>
+__device__ __forceinline__ void hop_pair(const typename Prec<T>::Vec* __restrict__ in,
+                                         const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, const Geom& G,
+                                         long long s, long long s_fwd, long long s_bwd, T ph_fwd, T ph_bwd, cx<T> (&acc)[12]) {
+    cx<T> psi[12], U[3][3], h[2][3], g[2][3];
+    // forward hop: U_mu(x) (1 - gamma_mu) phi(x + mu^)
+    load_spinor<T>(in, G.V, s_fwd, psi);
+    load_link<T, RECON>(gauge, G.V, MU, s, U);
+    project<T, MU, -1>(psi, ph_fwd, h);
+    mul_U(U, h, g);
+    accumulate<T, MU, -1>(g, acc);
+    // backward hop: U_mu(x - mu^)^dagger (1 + gamma_mu) phi(x - mu^)
+    load_spinor<T>(in, G.V, s_bwd, psi);
+    load_link<T, RECON>(gauge, G.V, MU, s_bwd, U);
+    project<T, MU, +1>(psi, ph_bwd, h);
+    mul_Udag(U, h, g);
+    accumulate<T, MU, +1>(g, acc);
+}
+
+template <typename T, int RECON, bool EPI>
+__global__ void __launch_bounds__(128) wilson_Q_kernel(typename Prec<T>::Vec* __restrict__ out,
+                                                       const typename Prec<T>::Vec* __restrict__ in,
+                                                       const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, Geom G,
+                                                       T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2,
+                                                       const typename Prec<T>::Vec* v2, T s3,
+                                                       const typename Prec<T>::Vec* v3) {
+    using Vec = typename Prec<T>::Vec;
+    constexpr int NV = Prec<T>::NV;
+    long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= G.V) return;
+    int x3 = (int)(s % G.L3);
+    long long r = s / G.L3;
+    int x2 = (int)(r % G.L2);
+    r /= G.L2;
+    int x1 = (int)(r % G.L1);
+    int x0 = (int)(r / G.L1);
+
+    cx<T> acc[12];
+#pragma unroll
+    for (int i = 0; i < 12; i++) acc[i] = {T(0), T(0)};
+
+    {
+        long long sf = (x0 == G.L0 - 1) ? s - (long long)(G.L0 - 1) * G.S0 : s + G.S0;
+        long long sb = (x0 == 0) ? s + (long long)(G.L0 - 1) * G.S0 : s - G.S0;
+        T pf = (x0 == G.L0 - 1) ? T(G.bc) : T(1);
+        T pb = (x0 == 0) ? T(G.bc) : T(1);
+        hop_pair<T, RECON, 0>(in, gauge, G, s, sf, sb, pf, pb, acc);
+    }
+    {
+        long long sf = (x1 == G.L1 - 1) ? s - (long long)(G.L1 - 1) * G.S1 : s + G.S1;
+        long long sb = (x1 == 0) ? s + (long long)(G.L1 - 1) * G.S1 : s - G.S1;
+        hop_pair<T, RECON, 1>(in, gauge, G, s, sf, sb, T(1), T(1), acc);
+    }
+    {
+        long long sf = (x2 == G.L2 - 1) ? s - (long long)(G.L2 - 1) * G.S2 : s + G.S2;
+        long long sb = (x2 == 0) ? s + (long long)(G.L2 - 1) * G.S2 : s - G.S2;
+        hop_pair<T, RECON, 2>(in, gauge, G, s, sf, sb, T(1), T(1), acc);
+    }
+    {
+        long long sf = (x3 == G.L3 - 1) ? s - (G.L3 - 1) : s + 1;
+        long long sb = (x3 == 0) ? s + (G.L3 - 1) : s - 1;
+        hop_pair<T, RECON, 3>(in, gauge, G, s, sf, sb, T(1), T(1), acc);
+    }
+
+    // out = gamma5 [ (4+m) phi(x) - 1/2 acc ]
+    cx<T> phi[12], res[12];
+    load_spinor<T>(in, G.V, s, phi);
+#pragma unroll
+    for (int i = 0; i < 12; i++) {
+        T sg = (i < 6) ? T(1) : T(-1);
+        res[i].re = sg * fma(T(-0.5), acc[i].re, mass_term * phi[i].re);
+        res[i].im = sg * fma(T(-0.5), acc[i].im, mass_term * phi[i].im);
+    }
+    Vec w[NV];
+    cx_to_words(res, w);
+    if (EPI) {
+        // out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3 ; read every v_i(x) before the store so out may alias them
+        T* wr = reinterpret_cast<T*>(w);
+        constexpr int NR = 24;
+#pragma unroll
+        for (int i = 0; i < NR; i++) wr[i] *= s0;
+        if (v1) {
+#pragma unroll
+            for (int p = 0; p < NV; p++) {
+                Vec a = v1[p * G.V + s];
+                const T* ar = reinterpret_cast<const T*>(&a);
+#pragma unroll
+                for (int k = 0; k < NR / NV; k++) wr[p * (NR / NV) + k] = fma(s1, ar[k], wr[p * (NR / NV) + k]);
+            }
+        }
+        if (v2) {
+#pragma unroll
+            for (int p = 0; p < NV; p++) {
+                Vec a = v2[p * G.V + s];
+                const T* ar = reinterpret_cast<const T*>(&a);
+#pragma unroll
+                for (int k = 0; k < NR / NV; k++) wr[p * (NR / NV) + k] = fma(s2, ar[k], wr[p * (NR / NV) + k]);
+            }
+        }
+        if (v3) {
+#pragma unroll
+            for (int p = 0; p < NV; p++) {
+                Vec a = v3[p * G.V + s];
+                const T* ar = reinterpret_cast<const T*>(&a);
+#pragma unroll
+                for (int k = 0; k < NR / NV; k++) wr[p * (NR / NV) + k] = fma(s3, ar[k], wr[p * (NR / NV) + k]);
+            }
+        }
+    }
+#pragma unroll
+    for (int p = 0; p < NV; p++) out[p * G.V + s] = w[p];
+}
+
+template <typename T, int RECON>
+int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
+             const void* v2, double s3, const void* v3) {
+    using Vec = typename Prec<T>::Vec;
+    using LVec = typename LinkLayout<T, RECON>::LVec;
+    Geom G;
+    G.L0 = ctx->dims[0]; G.L1 = ctx->dims[1]; G.L2 = ctx->dims[2]; G.L3 = ctx->dims[3];
+    G.V = ctx->V;
+    G.S2 = G.L3;
+    G.S1 = (long long)G.L2 * G.L3;
+    G.S0 = (long long)G.L1 * G.L2 * G.L3;
+    G.bc = ctx->bc;
+    const int threads = 128;
+    const unsigned blocks = (unsigned)((ctx->V + threads - 1) / threads);
+    if (epi)
+        wilson_Q_kernel<T, RECON, true><<<blocks, threads, 0, ctx->stream>>>(
+            (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(s0), T(s1), (const Vec*)v1, T(s2),
+            (const Vec*)v2, T(s3), (const Vec*)v3);
+    else
+        wilson_Q_kernel<T, RECON, false><<<blocks, threads, 0, ctx->stream>>>(
+            (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(1), T(0), nullptr, T(0), nullptr, T(0),
+            nullptr);
+    ND_LAUNCHED(ctx);
+    return ND_OK;
+}
+
+}  // namespace
+
+int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
+                double s2, const void* v2, double s3, const void* v3) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (!out || !in || out == in) return nd_fail(ctx, ND_ERR_BAD_ARG, "apply_Q: out/in null or aliased");
+    if (!ctx->gauge_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_Q: gauge field not set");
+    if (s1 == 0.0) v1 = nullptr;
+    if (s2 == 0.0) v2 = nullptr;
+    if (s3 == 0.0) v3 = nullptr;
+    if (v1 == in || v2 == in || v3 == in) {
+        // allowed (read-only), nothing to do
+    }
+#define ND_DISPATCH(T, R) return launch_Q<T, R>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3)
+    if (ctx->prec == 32) {
+        if (ctx->recon == 18) ND_DISPATCH(float, 18);
+        if (ctx->recon == 12) ND_DISPATCH(float, 12);
+        ND_DISPATCH(float, 8);
+    } else {
+        if (ctx->recon == 18) ND_DISPATCH(double, 18);
+        if (ctx->recon == 12) ND_DISPATCH(double, 12);
+        ND_DISPATCH(double, 8);
+    }
+#undef ND_DISPATCH
+}

@@ -1,0 +1,161 @@
+"""Parity of the CUDA Wilson-Dirac stencil (through the C-ABI) with the CPU oracle on the same seeded inputs.
+BASELINE.json configs 0-2; tolerances from north_star: rel-L2 <= 1e-12 (fp64), <= 1e-5 (fp32)."""
+import numpy as np
+import pytest
+
+from lattice_inputs import gauge_field, gaussian_spinor
+from oracle import su3, wilson, wilson_c
+from tests.gpu_common import TOL, make_context, rel_l2, round_to
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("bc", [-1, 1])
+@pytest.mark.parametrize("recon", [18, 12, 8])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_config0_4x4_haar(prec, recon, bc):
+    """BASELINE config 0: 4^4, m = 0.1, Haar links, Gaussian source, numpy oracle."""
+    dims = (4, 4, 4, 4)
+    ctx, U = make_context(dims, prec, recon, bc, "haar")
+    psi = round_to(gaussian_spinor(dims), prec)
+    x = ctx.pack_spinor(psi)
+    y = ctx.new_spinor()
+    ctx.apply_Q(y, x, 0.1)
+    got = ctx.unpack_spinor(y)
+    ref = wilson.apply_Q(psi, U, 0.1, bc)
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_config0_free_field_plane_wave(prec, recon):
+    """Unit links: Q on a plane wave equals the closed form gamma5 (M + i sum gamma_mu sin p_mu) (pin P3), checked on
+    the CUDA path directly (no oracle in the loop)."""
+    dims = (8, 4, 6, 4)
+    ctx, U = make_context(dims, prec, recon, -1, "unit")
+    g, g5 = wilson.gamma_matrices()
+    n = (1, 2, 5, 3)
+    p = [(2 * n[0] + 1) * np.pi / dims[0]] + [2 * np.pi * n[i] / dims[i] for i in (1, 2, 3)]
+    grids = np.meshgrid(*[np.arange(d) for d in dims], indexing="ij")
+    phase = np.exp(1j * sum(p[i] * grids[i] for i in range(4)))
+    rng = np.random.default_rng(5)
+    w = rng.standard_normal((4, 3)) + 1j * rng.standard_normal((4, 3))
+    psi = round_to(phase[..., None, None] * w, prec)
+    m = -1.6
+    M = 4 + m - sum(np.cos(p))
+    Dp = M * np.eye(4) + 1j * sum(np.sin(p[mu]) * g[mu] for mu in range(4))
+    ref = phase[..., None, None] * (g5 @ Dp @ w)
+    x = ctx.pack_spinor(psi)
+    y = ctx.new_spinor()
+    ctx.apply_Q(y, x, m)
+    assert rel_l2(ctx.unpack_spinor(y), ref) <= (1e-12 if prec == 64 else 2e-6)
+
+
+def test_recon8_flags_unit_links():
+    import paper_1010_5636_b200 as nd
+
+    dims = (4, 4, 4, 4)
+    ctx = nd.Context(dims, prec=64, recon=8)
+    with pytest.raises(nd.NDError) as e:
+        ctx.set_gauge(gauge_field(dims, "unit"))
+    assert e.value.code == -4
+
+
+def test_set_gauge_rejects_non_su3():
+    import paper_1010_5636_b200 as nd
+
+    dims = (4, 4, 4, 4)
+    U = gauge_field(dims, "haar")
+    U[2, 1, 2, 3, 0] *= 1.001
+    ctx = nd.Context(dims, prec=64, recon=12)
+    with pytest.raises(nd.NDError) as e:
+        ctx.set_gauge(U)
+    assert e.value.code == -3
+    y = ctx.new_spinor()
+    with pytest.raises(nd.NDError) as e:
+        ctx.apply_Q(y, ctx.new_spinor(), 0.1)     # gauge not set after the failure
+    assert e.value.code == -2
+
+
+@pytest.mark.parametrize("dims", [(6, 4, 2, 10), (4, 6, 12, 2), (2, 2, 2, 2), (10, 6, 6, 6)])
+@pytest.mark.parametrize("recon", [12, 8])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_ragged_lattices(prec, recon, dims):
+    """Extents that are not multiples of the warp / tile sizes, extent-2 directions (forward and backward neighbour
+    coincide), and a volume with a ragged last block."""
+    ctx, U = make_context(dims, prec, recon, -1, "smooth", eps=0.3)
+    psi = round_to(gaussian_spinor(dims), prec)
+    y = ctx.new_spinor()
+    ctx.apply_Q(y, ctx.pack_spinor(psi), -1.6)
+    ref = wilson_c.apply_Q(psi, U, -1.6, -1)
+    assert rel_l2(ctx.unpack_spinor(y), ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("recon", [12, 8])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_config1_16c32(prec, recon):
+    """BASELINE config 1: 16^3 x 32, m = -1.6, exp(0.3 i H) links, both compressions, both precisions (C oracle)."""
+    dims = (32, 16, 16, 16)
+    ctx, U = make_context(dims, prec, recon, -1, "smooth", eps=0.3)
+    psi = round_to(gaussian_spinor(dims), prec)
+    x = ctx.pack_spinor(psi)
+    y = ctx.new_spinor()
+    ctx.apply_Q(y, x, -1.6)
+    ref = wilson_c.apply_Q(psi, U, -1.6, -1)
+    assert rel_l2(ctx.unpack_spinor(y), ref) <= TOL[prec]
+    # Q^2 through the temporary
+    z, t = ctx.new_spinor(), ctx.new_spinor()
+    ctx.apply_Q2(z, x, t, -1.6)
+    ref2 = wilson_c.apply_Q(ref, U, -1.6, -1)
+    assert rel_l2(ctx.unpack_spinor(z), ref2) <= 2 * TOL[prec]
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_fused_epilogue(prec):
+    """out = s0 Q(in) + s1 v1 + s2 v2 + s3 v3 with out aliasing v2 (the Clenshaw step)."""
+    dims = (8, 4, 4, 8)
+    ctx, U = make_context(dims, prec, 12, -1, "smooth")
+    f = [round_to(gaussian_spinor(dims, seed=10 + i), prec) for i in range(4)]
+    d = [ctx.pack_spinor(a) for a in f]
+    s0, s1, s2, s3 = 0.37, -1.2, -1.0, 0.81
+    ctx.apply_Q_axpbycz(d[2], d[0], -1.6, s0, s1, d[1], s2, d[2], s3, d[3])
+    ref = s0 * wilson.apply_Q(f[0], U, -1.6, -1) + s1 * f[1] + s2 * f[2] + s3 * f[3]
+    assert rel_l2(ctx.unpack_spinor(d[2]), ref) <= TOL[prec]
+    # null vectors with zero scalars
+    out = ctx.new_spinor()
+    ctx.apply_Q_axpbycz(out, d[0], -1.6, 2.0)
+    assert rel_l2(ctx.unpack_spinor(out), 2.0 * wilson.apply_Q(f[0], U, -1.6, -1)) <= TOL[prec]
+
+
+def test_aliasing_is_rejected():
+    import paper_1010_5636_b200 as nd
+
+    ctx, _ = make_context((4, 4, 4, 4), 64, 12)
+    x = ctx.new_spinor()
+    with pytest.raises(nd.NDError) as e:
+        ctx.apply_Q(x, x, 0.1)
+    assert e.value.code == -1
+
+
+@pytest.mark.parametrize("kind", ["haar", "smooth"])
+@pytest.mark.parametrize("recon", [18, 12, 8])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_gauge_round_trip(prec, recon, kind):
+    """reconstruct(compress(U)) = U through nd_set_gauge / nd_get_gauge (pin P6 on the CUDA side)."""
+    dims = (4, 6, 4, 8)
+    ctx, U = make_context(dims, prec, recon, -1, kind)
+    back = ctx.get_gauge()
+    tol = {64: {18: 1e-15, 12: 1e-14, 8: 1e-11}, 32: {18: 1e-7, 12: 3e-7, 8: 2e-5}}[prec][recon]
+    assert rel_l2(back, U) <= tol
+    st = ctx.gauge_stats()
+    assert st[0] < (1e-12 if prec == 64 else 1e-6) and abs(st[2] - su3.recon8_min_N(U)) < 1e-6
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_pack_unpack_round_trip(prec):
+    dims = (4, 6, 2, 8)
+    ctx, _ = make_context(dims, prec, 12)
+    psi = round_to(gaussian_spinor(dims), prec)
+    assert np.array_equal(ctx.unpack_spinor(ctx.pack_spinor(psi)), psi)
+    assert np.array_equal(ctx.unpack_spinor(ctx.pack_spinor(psi.astype(np.complex64)), prec=32),
+                          psi.astype(np.complex64))
