@@ -138,6 +138,10 @@ ND_API int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor,
 ND_API int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, double m, double tol, int maxit,
                         unsigned long long seed, void* u_out, double* nu, double* resid, void* work,
                         long long* stats);
+/* Host utility (no GPU) used by nd_lowmodes_compute for the small dense problems of PAPER.md:L81: eigendecomposition
+ * of a k x k Hermitian matrix a (row-major, complex as (re, im) pairs; only its Hermitian part is used) by the cyclic
+ * Jacobi method: a = Z diag(w) Z^dagger, w[k] ascending, eigenvector j in COLUMN j of z (row-major, k*k complex). */
+ND_API int nd_heev(int k, const double* a, double* w, double* z);
 
 /* ------------------------------------------------------------------------------------------------ BLAS-1
  * Spinor-field vector operations (device SoA).  a = (re, im).

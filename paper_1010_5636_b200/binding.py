@@ -50,6 +50,7 @@ SIGNATURES = {
     "nd_apply_DN": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_vp, _c_int]),
     "nd_lowmodes_compute": (_c_int, [_c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_ull, _c_vp, _pd, _pd,
                                      _c_vp, ctypes.POINTER(_c_ll)]),
+    "nd_heev": (_c_int, [_c_int, _pd, _pd, _pd]),
     "nd_axpy": (_c_int, [_c_vp, _pd, _c_vp, _c_vp]),
     "nd_scale": (_c_int, [_c_vp, _pd, _c_vp]),
     "nd_copy": (_c_int, [_c_vp, _c_vp, _c_vp]),
@@ -99,6 +100,21 @@ def cheb_coeffs(n, eps):
     if rc != ND_OK:
         raise NDError(rc, "nd_cheb_coeffs")
     return c, delta.value
+
+
+def heev(a):
+    """nd_heev: Hermitian eigendecomposition (cyclic Jacobi) of a k x k complex matrix -> (w ascending, Z columns) -
+    host utility, needs no GPU."""
+    lib = load_library()
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    k = a.shape[0]
+    assert a.shape == (k, k)
+    w = np.zeros(k)
+    z = np.zeros((k, k), dtype=np.complex128)
+    rc = lib.nd_heev(k, a.view(np.float64).ctypes.data_as(_pd), w.ctypes.data_as(_pd), z.view(np.float64).ctypes.data_as(_pd))
+    if rc != ND_OK:
+        raise NDError(rc, "nd_heev")
+    return w, z
 
 
 def _ptr(x):

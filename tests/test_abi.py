@@ -1,0 +1,117 @@
+"""Host-side checks of the C-ABI boundary that need no GPU: the library loads, exports every symbol that
+include/nd_b200.h declares, the binding covers exactly those symbols, the two host utilities (nd_cheb_coeffs, nd_heev)
+agree with independent computations, and the product fails loudly (never falls back) without a CUDA device."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "nd_b200.h")
+
+
+def declared_symbols():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"ND_API\s+[\w\s\*]+?\b(nd_\w+)\s*\(", text)))
+
+
+def test_header_declares_the_boundary_calls():
+    names = declared_symbols()
+    for must in ("nd_create", "nd_set_gauge", "nd_apply_Q", "nd_apply_Q2", "nd_apply_DN", "nd_apply_sign", "nd_axpy",
+                 "nd_dot", "nd_norm2", "nd_block_dot", "nd_block_axpy", "nd_lowmodes_compute", "nd_pack_spinor"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol():
+    import paper_1010_5636_b200 as nd
+
+    lib = nd.load_library()
+    raw = ctypes.CDLL(nd.LIB_PATH)
+    for name in declared_symbols():
+        assert hasattr(raw, name), f"{name} declared in nd_b200.h but not exported"
+    assert sorted(nd.SIGNATURES) == declared_symbols()
+    assert lib is nd.load_library()
+
+
+def test_only_declared_symbols_are_exported():
+    import paper_1010_5636_b200 as nd
+
+    out = subprocess.run(["nm", "-D", "--defined-only", nd.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    exported = sorted(l.split()[-1] for l in out.splitlines() if " T " in l and l.split()[-1].startswith("nd_"))
+    assert exported == declared_symbols()
+
+
+def test_cheb_coeffs_matches_independent_fit():
+    """nd_cheb_coeffs (library, long double DCT) vs numpy's Chebyshev interpolation of y^{-1/2} on [eps, 1] and the
+    delta table of SURVEY.md 8(c)-A7."""
+    import paper_1010_5636_b200 as nd
+    from numpy.polynomial import chebyshev as C
+
+    for n, eps, dref in ((100, 0.01, 5.4e-10), (100, 0.002, 5.9e-5), (200, 0.002, 5.6e-9)):
+        c, delta = nd.cheb_coeffs(n, eps)
+        ref = C.chebinterpolate(lambda z: 1.0 / np.sqrt(((1 - eps) * z + 1 + eps) / 2), n)
+        assert np.abs(c - ref).max() < 1e-12 * np.abs(ref).max()
+        assert abs(delta / dref - 1) < 0.05
+    assert nd.load_library().nd_cheb_coeffs(5, 1.5, None, None) == -1
+
+
+def test_heev_matches_lapack():
+    import paper_1010_5636_b200 as nd
+
+    rng = np.random.default_rng(3)
+    for k in (1, 2, 7, 28, 64):
+        a = rng.standard_normal((k, k)) + 1j * rng.standard_normal((k, k))
+        a = a + a.conj().T
+        w, z = nd.heev(a)
+        assert np.abs(w - np.linalg.eigvalsh(a)).max() < 1e-12 * max(1.0, np.abs(a).max() * k)
+        assert np.abs(z.conj().T @ z - np.eye(k)).max() < 1e-12
+        assert np.abs(a @ z - z * w).max() < 1e-11 * max(1.0, np.abs(a).max() * k)
+    # degenerate spectrum and an already diagonal matrix
+    w, z = nd.heev(np.diag([2.0, 1.0, 1.0, 2.0, -3.0]).astype(np.complex128))
+    assert np.allclose(w, [-3, 1, 1, 2, 2]) and np.abs(z.conj().T @ z - np.eye(5)).max() < 1e-15
+
+
+def test_no_cpu_fallback_without_a_device():
+    """Without a CUDA device nd_create must fail with ND_ERR_CUDA and Context() must raise."""
+    import torch
+
+    import paper_1010_5636_b200 as nd
+
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    lib = nd.load_library()
+    h = ctypes.c_void_p()
+    dims = (ctypes.c_int * 4)(4, 4, 4, 4)
+    assert lib.nd_create(ctypes.byref(h), dims, 64, 12, -1, 0, None) == -5 and not h.value
+    with pytest.raises(nd.NDError):
+        nd.Context((4, 4, 4, 4))
+    # null / bad arguments are reported, not crashed on
+    assert lib.nd_create(None, dims, 64, 12, -1, 0, None) == -1
+    assert lib.nd_create(ctypes.byref(h), dims, 16, 12, -1, 0, None) == -1
+    assert lib.nd_apply_Q(None, None, None, 0.0) == -1
+    assert lib.nd_last_error(None) == b"null context"
+
+
+def test_product_never_imports_the_oracle():
+    """The CUDA path and the oracle share no code: nothing under paper_1010_5636_b200/ mentions oracle/, and
+    importing the package does not pull the oracle in."""
+    pkg = os.path.join(ROOT, "paper_1010_5636_b200")
+    for dirpath, _, files in os.walk(pkg):
+        if os.path.basename(dirpath) in ("build", "__pycache__"):
+            continue
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
+                assert "wilson_ref" not in text, f
+    code = "import sys; import paper_1010_5636_b200; assert not any(m == 'oracle' or m.startswith('oracle.') for m in sys.modules)"
+    subprocess.run([sys.executable, "-c", code], cwd=ROOT, check=True)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_1010_5636_b200" not in text.replace("`paper_1010_5636_b200/`", ""), f

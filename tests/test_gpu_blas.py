@@ -1,0 +1,91 @@
+"""Parity of the BLAS-1 and block (low-mode projection) kernels with numpy on the same seeded inputs
+(pin P13: fp32 data with fp64 accumulation agrees with the fp64 result to ~1e-7)."""
+import numpy as np
+import pytest
+
+from lattice_inputs import gaussian_spinor
+from tests.gpu_common import make_context, rel_l2, round_to
+
+pytestmark = pytest.mark.gpu
+
+DIMS = [(4, 4, 4, 4), (6, 4, 2, 10), (10, 6, 6, 6), (16, 8, 8, 8)]
+
+
+@pytest.mark.parametrize("dims", DIMS)
+@pytest.mark.parametrize("prec", [64, 32])
+def test_axpy_scale_copy_gamma5(prec, dims):
+    from oracle import wilson
+
+    ctx, _ = make_context(dims, prec, 12, -1, "smooth")
+    tol = 1e-14 if prec == 64 else 2e-7
+    a = round_to(gaussian_spinor(dims, seed=1), prec)
+    b = round_to(gaussian_spinor(dims, seed=2), prec)
+    x, y = ctx.pack_spinor(a), ctx.pack_spinor(b)
+    alpha = 0.37 - 1.21j
+    ctx.axpy(alpha, x, y)
+    assert rel_l2(ctx.unpack_spinor(y), alpha * a + b) <= tol
+    ctx.scale(-0.5 + 2j, x)
+    assert rel_l2(ctx.unpack_spinor(x), (-0.5 + 2j) * a) <= tol
+    z = ctx.new_spinor()
+    ctx.copy(z, y)
+    assert np.array_equal(ctx.unpack_spinor(z), ctx.unpack_spinor(y))
+    ctx.gamma5(z, z)
+    assert rel_l2(ctx.unpack_spinor(z), wilson.apply_gamma5(alpha * a + b)) <= tol
+
+
+@pytest.mark.parametrize("dims", DIMS)
+@pytest.mark.parametrize("prec", [64, 32])
+def test_dot_norm(prec, dims):
+    ctx, _ = make_context(dims, prec, 12, -1, "smooth")
+    a = round_to(gaussian_spinor(dims, seed=1), prec)
+    b = round_to(gaussian_spinor(dims, seed=2), prec)
+    x, y = ctx.pack_spinor(a), ctx.pack_spinor(b)
+    ref = np.vdot(a.ravel(), b.ravel())
+    # fp64 accumulation of exactly representable products: the rounded inputs give the fp64 result in both precisions
+    assert abs(ctx.dot(x, y) - ref) <= 1e-13 * np.linalg.norm(a) * np.linalg.norm(b)
+    assert abs(ctx.norm2(x) - np.vdot(a.ravel(), a.ravel()).real) <= 1e-13 * np.linalg.norm(a) ** 2
+    # run-to-run bitwise reproducibility (no atomics in the reduction)
+    assert ctx.dot(x, y) == ctx.dot(x, y)
+
+
+@pytest.mark.parametrize("l", [1, 3, 20, 50])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_block_dot_and_block_axpy(prec, l):
+    dims = (6, 4, 6, 10)
+    ctx, _ = make_context(dims, prec, 12, -1, "smooth")
+    vs = [round_to(gaussian_spinor(dims, seed=100 + k), prec) for k in range(l)]
+    xh = round_to(gaussian_spinor(dims, seed=7), prec)
+    V = ctx.new_spinor(l)
+    for k in range(l):
+        ctx.pack_spinor(vs[k], out=V[k])
+    x = ctx.pack_spinor(xh)
+    got = ctx.block_dot(V, x)
+    ref = np.array([np.vdot(v.ravel(), xh.ravel()) for v in vs])
+    assert np.abs(got - ref).max() <= 1e-13 * np.linalg.norm(xh) * max(np.linalg.norm(v) for v in vs)
+    rng = np.random.default_rng(5)
+    a = rng.standard_normal(l) + 1j * rng.standard_normal(l)
+    ctx.block_axpy(a, V, x)
+    refy = xh + sum(a[k] * vs[k] for k in range(l))
+    assert rel_l2(ctx.unpack_spinor(x), refy) <= (1e-14 if prec == 64 else 3e-7)
+    # bad block sizes are rejected
+    import paper_1010_5636_b200 as nd
+    out = np.zeros(2)
+    rc = ctx.lib.nd_block_dot(ctx._h, 0, V.data_ptr(), x.data_ptr(), out.ctypes.data_as(nd.binding._pd))
+    assert rc == -1 and b"block_dot" in ctx.lib.nd_last_error(ctx._h)
+
+
+def test_gaussian_moments_and_determinism():
+    ctx, _ = make_context((8, 8, 8, 8), 32, 12, -1, "smooth")
+    x, y = ctx.new_spinor(), ctx.new_spinor()
+    ctx.gaussian(x, 11)
+    ctx.gaussian(y, 11)
+    ctx.synchronize()
+    a = ctx.unpack_spinor(x)
+    assert np.array_equal(a, ctx.unpack_spinor(y))
+    r = np.concatenate([a.real.ravel(), a.imag.ravel()])
+    n = r.size
+    assert abs(r.mean()) < 5 / np.sqrt(n) and abs(r.var() - 1) < 5 * np.sqrt(2 / n)
+    assert abs((r ** 4).mean() - 3) < 0.1
+    ctx.gaussian(y, 12)
+    b = ctx.unpack_spinor(y)
+    assert abs(np.vdot(a.ravel(), b.ravel())) < 6 * np.sqrt(n)
