@@ -263,14 +263,31 @@ def run_b200(args):
     prec, recon, n, l = args.prec, args.recon, args.degree, args.lowmodes
     peak, peak_src = load_peaks()
 
-    U64 = gauge_field(dims, "haar")                       # BASELINE config 2: Haar-random links, seeded
+    # BASELINE config 2: Haar-random links, seeded (configs 1, 3, 4: --field smooth)
+    U64 = gauge_field(dims, args.field, eps=args.field_eps)
     ctx = nd.Context(dims, prec=prec, recon=recon, bc_time=-1, device=local)
     ctx.set_gauge(U64.astype(np.complex64) if prec == 32 else U64)
     V = ctx.V
     qnorm = abs(4.0 + M_KERNEL) + 4.0
     c, delta = nd.cheb_coeffs(n, args.eps)
     ctx.set_sign_poly(c, args.eps, qnorm, M_KERNEL)
-    modes, nu = build_modes(ctx, l)
+    eig = None
+    if args.eigensolve and l > 0:
+        # BASELINE config 4: the low modes come from the library's own eigen-solver (a10), timed on the host clock
+        # (it synchronises for its small dense problems); eps then follows DESIGN.md R11.
+        ctx.synchronize()
+        t0 = time.perf_counter()
+        modes, nu, resid, st = ctx.lowmodes_compute(l, M_KERNEL, tol=args.eig_tol, maxit=60, lextra=max(8, l // 4),
+                                                    degree=args.eig_degree)
+        ctx.synchronize()
+        eig = {"seconds": time.perf_counter() - t0, "l": l, "tol_Q2_residual": args.eig_tol, "converged": st["converged"],
+               "outer_iterations": st["iterations"], "q_stencils": st["stencils"], "max_residue_Q": float(resid.max()),
+               "nu2_min": float((nu ** 2).min()), "nu2_max": float((nu ** 2).max())}
+        args.eps = 0.99 * float((nu ** 2).max()) / qnorm ** 2
+        c, delta = nd.cheb_coeffs(n, args.eps)
+        ctx.set_sign_poly(c, args.eps, qnorm, M_KERNEL)
+    else:
+        modes, nu = build_modes(ctx, l)
     ctx.set_lowmodes(modes, nu)
     eta, out, work = ctx.new_spinor(), ctx.new_spinor(), ctx.new_spinor(3)
     ctx.gaussian(eta, 5636 + rank)                        # replicas: a different source per rank
@@ -343,7 +360,7 @@ def run_b200(args):
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
-        "config": {"workload": f"D_N apply (eq. 2.4+2.11) on {args.lattice}, Haar SU(3) links, m=-1.6, recon {recon}, "
+        "config": {"workload": f"D_N apply (eq. 2.4+2.11) on {args.lattice}, {args.field} SU(3) links, m=-1.6, recon {recon}, "
                                f"degree n={n} (2n+1={stencils} Q stencils), l={l} projected modes, CUDA graph",
                    "lattice": args.lattice, "sites": V, "recon": recon, "degree": n, "eps": args.eps, "delta": delta,
                    "lowmodes": l, "replicas": world, "parallelism": f"replicas x{world}",
@@ -358,6 +375,8 @@ def run_b200(args):
         "q_kernel": qk,
         "cpu_baseline": cpu,
     }
+    if eig is not None:
+        line["eigensolve"] = eig
     print(json.dumps(line))
     if world > 1:
         dist.barrier()
@@ -396,6 +415,11 @@ def main():
     ap.add_argument("--degree", type=int, default=100)
     ap.add_argument("--eps", type=float, default=0.002)
     ap.add_argument("--lowmodes", type=int, default=8)
+    ap.add_argument("--field", default="haar", choices=["haar", "smooth"], help="gauge field recipe (DESIGN.md section 4)")
+    ap.add_argument("--field-eps", type=float, default=0.25, help="eps of U = exp(i eps H) for --field smooth")
+    ap.add_argument("--eigensolve", action="store_true", help="low modes from nd_lowmodes_compute (timed), eps by R11")
+    ap.add_argument("--eig-tol", type=float, default=2e-4)
+    ap.add_argument("--eig-degree", type=int, default=80)
     ap.add_argument("--quick", action="store_true", help="time only the line's own Q-kernel variant")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -19,6 +19,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false"]
 FLAGS = [f for f in FLAGS if f != "--use_fast_math=false"]   # IEEE arithmetic: never fast-math
+FLAGS += os.environ.get("ND_NVCC_EXTRA", "").split()        # tuning sweeps only (e.g. -DND_MINB32=6)
 
 
 def _deps():

@@ -24,18 +24,25 @@ template <typename T> __device__ __forceinline__ void third_row(cx<T> (&U)[3][3]
     U[2][2] = cj(U[0][0] * U[1][1] - U[0][1] * U[1][0]);
 }
 
+// the NL stored words of link (mu, s), as they sit in memory
 template <typename T, int RECON>
-__device__ __forceinline__ void load_link(const typename LinkLayout<T, RECON>::LVec* __restrict__ g, long long V, int mu,
-                                          long long s, cx<T> (&U)[3][3]) {
+__device__ __forceinline__ void load_link_words(const typename LinkLayout<T, RECON>::LVec* __restrict__ g, long long V, int mu,
+                                                long long s, typename LinkLayout<T, RECON>::LVec (&w)[LinkLayout<T, RECON>::NL]) {
+    using LL = LinkLayout<T, RECON>;
+    const typename LL::LVec* base = g + (long long)mu * LL::NL * V + s;
+#pragma unroll
+    for (int p = 0; p < LL::NL; p++) w[p] = ldg_vec(base + p * V);
+}
+
+// the 3x3 matrix from the stored words, in registers
+template <typename T, int RECON>
+__device__ __forceinline__ void reconstruct_link(const typename LinkLayout<T, RECON>::LVec (&w)[LinkLayout<T, RECON>::NL],
+                                                 cx<T> (&U)[3][3]) {
     using LL = LinkLayout<T, RECON>;
     constexpr int W = sizeof(typename LL::LVec) / sizeof(T);
     T r[LL::NL * W];
-    const typename LL::LVec* base = g + (long long)mu * LL::NL * V + s;
 #pragma unroll
-    for (int p = 0; p < LL::NL; p++) {
-        typename LL::LVec v = ldg_vec(base + p * V);
-        unpack_reals<T>(v, r + p * W);
-    }
+    for (int p = 0; p < LL::NL; p++) unpack_reals<T>(w[p], r + p * W);
     if (RECON == 18) {
 #pragma unroll
         for (int i = 0; i < 3; i++)
@@ -71,3 +78,11 @@ __device__ __forceinline__ void load_link(const typename LinkLayout<T, RECON>::L
     }
 }
 
+
+template <typename T, int RECON>
+__device__ __forceinline__ void load_link(const typename LinkLayout<T, RECON>::LVec* __restrict__ g, long long V, int mu,
+                                          long long s, cx<T> (&U)[3][3]) {
+    typename LinkLayout<T, RECON>::LVec w[LinkLayout<T, RECON>::NL];
+    load_link_words<T, RECON>(g, V, mu, s, w);
+    reconstruct_link<T, RECON>(w, U);
+}

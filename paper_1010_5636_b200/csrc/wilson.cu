@@ -111,15 +111,64 @@ __device__ __forceinline__ void hop_pair(const typename Prec<T>::Vec* __restrict
     accumulate<T, MU, +1>(g, acc);
 }
 
+// out(x) = gamma5 [ (4+m) phi(x) - 1/2 acc ], optionally followed by the fused vector update
+// out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3 (every v_i(x) is read before the store, so out may alias them)
+template <typename T, bool EPI>
+__device__ __forceinline__ void finish_site(typename Prec<T>::Vec* __restrict__ out, long long V, long long s,
+                                            const cx<T> (&phi)[12], const cx<T> (&acc)[12], T mass_term, T s0, T s1,
+                                            const typename Prec<T>::Vec* v1, T s2, const typename Prec<T>::Vec* v2, T s3,
+                                            const typename Prec<T>::Vec* v3) {
+    using Vec = typename Prec<T>::Vec;
+    constexpr int NV = Prec<T>::NV;
+    cx<T> res[12];
+#pragma unroll
+    for (int i = 0; i < 12; i++) {
+        T sg = (i < 6) ? T(1) : T(-1);
+        res[i].re = sg * fma(T(-0.5), acc[i].re, mass_term * phi[i].re);
+        res[i].im = sg * fma(T(-0.5), acc[i].im, mass_term * phi[i].im);
+    }
+    Vec w[NV];
+    cx_to_words(res, w);
+    if (EPI) {
+        T* wr = reinterpret_cast<T*>(w);
+        constexpr int NR = 24;
+#pragma unroll
+        for (int i = 0; i < NR; i++) wr[i] *= s0;
+        const Vec* vs[3] = {v1, v2, v3};
+        const T ss[3] = {s1, s2, s3};
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            if (vs[j]) {
+#pragma unroll
+                for (int p = 0; p < NV; p++) {
+                    Vec a = vs[j][p * V + s];
+                    const T* ar = reinterpret_cast<const T*>(&a);
+#pragma unroll
+                    for (int k = 0; k < NR / NV; k++) wr[p * (NR / NV) + k] = fma(ss[j], ar[k], wr[p * (NR / NV) + k]);
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int p = 0; p < NV; p++) out[p * V + s] = w[p];
+}
+
+#ifndef ND_MINB32
+#define ND_MINB32 5
+#endif
+#ifndef ND_MINB64
+#define ND_MINB64 3
+#endif
+// resident CTAs per SM the register allocation is tuned for (fp32 / fp64)
+template <typename T> constexpr int q_min_blocks() { return sizeof(T) == 4 ? ND_MINB32 : ND_MINB64; }
+
 template <typename T, int RECON, bool EPI>
-__global__ void __launch_bounds__(128) wilson_Q_kernel(typename Prec<T>::Vec* __restrict__ out,
+__global__ void __launch_bounds__(128, q_min_blocks<T>()) wilson_Q_kernel(typename Prec<T>::Vec* __restrict__ out,
                                                        const typename Prec<T>::Vec* __restrict__ in,
                                                        const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, Geom G,
                                                        T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2,
                                                        const typename Prec<T>::Vec* v2, T s3,
                                                        const typename Prec<T>::Vec* v3) {
-    using Vec = typename Prec<T>::Vec;
-    constexpr int NV = Prec<T>::NV;
     long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= G.V) return;
     int x3 = (int)(s % G.L3);
@@ -156,53 +205,9 @@ __global__ void __launch_bounds__(128) wilson_Q_kernel(typename Prec<T>::Vec* __
         hop_pair<T, RECON, 3>(in, gauge, G, s, sf, sb, T(1), T(1), acc);
     }
 
-    // out = gamma5 [ (4+m) phi(x) - 1/2 acc ]
-    cx<T> phi[12], res[12];
+    cx<T> phi[12];
     load_spinor<T>(in, G.V, s, phi);
-#pragma unroll
-    for (int i = 0; i < 12; i++) {
-        T sg = (i < 6) ? T(1) : T(-1);
-        res[i].re = sg * fma(T(-0.5), acc[i].re, mass_term * phi[i].re);
-        res[i].im = sg * fma(T(-0.5), acc[i].im, mass_term * phi[i].im);
-    }
-    Vec w[NV];
-    cx_to_words(res, w);
-    if (EPI) {
-        // out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3 ; read every v_i(x) before the store so out may alias them
-        T* wr = reinterpret_cast<T*>(w);
-        constexpr int NR = 24;
-#pragma unroll
-        for (int i = 0; i < NR; i++) wr[i] *= s0;
-        if (v1) {
-#pragma unroll
-            for (int p = 0; p < NV; p++) {
-                Vec a = v1[p * G.V + s];
-                const T* ar = reinterpret_cast<const T*>(&a);
-#pragma unroll
-                for (int k = 0; k < NR / NV; k++) wr[p * (NR / NV) + k] = fma(s1, ar[k], wr[p * (NR / NV) + k]);
-            }
-        }
-        if (v2) {
-#pragma unroll
-            for (int p = 0; p < NV; p++) {
-                Vec a = v2[p * G.V + s];
-                const T* ar = reinterpret_cast<const T*>(&a);
-#pragma unroll
-                for (int k = 0; k < NR / NV; k++) wr[p * (NR / NV) + k] = fma(s2, ar[k], wr[p * (NR / NV) + k]);
-            }
-        }
-        if (v3) {
-#pragma unroll
-            for (int p = 0; p < NV; p++) {
-                Vec a = v3[p * G.V + s];
-                const T* ar = reinterpret_cast<const T*>(&a);
-#pragma unroll
-                for (int k = 0; k < NR / NV; k++) wr[p * (NR / NV) + k] = fma(s3, ar[k], wr[p * (NR / NV) + k]);
-            }
-        }
-    }
-#pragma unroll
-    for (int p = 0; p < NV; p++) out[p * G.V + s] = w[p];
+    finish_site<T, EPI>(out, G.V, s, phi, acc, mass_term, s0, s1, v1, s2, v2, s3, v3);
 }
 
 template <typename T, int RECON>
