@@ -283,6 +283,10 @@ def run_b200(args):
         eig = {"seconds": time.perf_counter() - t0, "l": l, "tol_Q2_residual": args.eig_tol, "converged": st["converged"],
                "outer_iterations": st["iterations"], "q_stencils": st["stencils"], "max_residue_Q": float(resid.max()),
                "nu2_min": float((nu ** 2).min()), "nu2_max": float((nu ** 2).max())}
+        rest = np.sqrt(np.maximum(st["theta_rest"], 0.0))
+        kappa, bound, _ = nd.projector_error(nu, resid, np.concatenate([rest, -rest]))     # eq. 2.9-2.10
+        eig["kappa_pm"] = [float(kappa[0]), float(kappa[1])]
+        eig["projector_bound_pm"] = [float(b) if np.isfinite(b) else None for b in bound]
         args.eps = 0.99 * float((nu ** 2).max()) / qnorm ** 2
         c, delta = nd.cheb_coeffs(n, args.eps)
         ctx.set_sign_poly(c, args.eps, qnorm, M_KERNEL)

@@ -136,8 +136,19 @@ ND_API int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor,
  * residuals of Q^2 are <= tol or after maxit outer iterations (ND_ERR_NO_CONVERGENCE, results still filled).
  * stats (may be NULL): [0] outer iterations, [1] stencil applications. */
 ND_API int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, double m, double tol, int maxit,
-                        unsigned long long seed, void* u_out, double* nu, double* resid, void* work,
-                        long long* stats);
+                        unsigned long long seed, void* u_out, double* nu, double* resid, double* theta_rest,
+                        void* work, long long* stats);
+/* theta_rest (may be NULL): the lextra Ritz values of Q^2 of the guard vectors from the last Rayleigh-Ritz step,
+ * ascending - upper estimates of the next eigenvalues of Q^2 above the l returned ones (input of nd_projector_error).
+ *
+ * Error control of the projectors (host utility, no GPU; eq. 2.8-2.10): from the Ritz values nu[l],
+ * the residues rho[l] (eq. 2.8) and estimates rest[nrest] of the eigenvalues of Q outside the low-mode space, compute
+ *   d_k      = distance of nu_k from {rest} and from the Ritz values of the opposite sign
+ *   kappa[0] = kappa_+, kappa[1] = kappa_-,  kappa_+-^2 = sum_{+-nu_k > 0} rho_k^2 / d_k^2              (2.9)
+ *   bound[i] = kappa (1 + 2 kappa) / (1 - 2 kappa (1 + 2 kappa))  >= || P_+- - (P_+-)_exact ||          (2.10)
+ * bound[i] = +infinity when the denominator is not positive.  d (may be NULL) receives the l distances. */
+ND_API int nd_projector_error(int l, const double* nu, const double* rho, int nrest, const double* rest, double kappa[2],
+                              double bound[2], double* d);
 /* Host utility (no GPU) used by nd_lowmodes_compute for the small dense problems of PAPER.md:L81: eigendecomposition
  * of a k x k Hermitian matrix a (row-major, complex as (re, im) pairs; only its Hermitian part is used) by the cyclic
  * Jacobi method: a = Z diag(w) Z^dagger, w[k] ascending, eigenvector j in COLUMN j of z (row-major, k*k complex). */

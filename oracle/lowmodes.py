@@ -73,3 +73,34 @@ def approximate_low_space(Q, shape, l, qnorm, cut, degree=24, sweeps=3, seed=11)
     for _ in range(sweeps):
         V = orthonormalise([filt(v) for v in V])
     return V
+
+
+# ----------------------------------------------------------------------------- error control, eq. 2.8-2.10
+def distances_d(nu, spectrum_rest):
+    """d_k of PAPER.md:L90: the distance of nu_k from the spectrum of Q in the subspace orthogonal to the range of
+    (P_+)_exact if nu_k > 0, of (P_-)_exact if nu_k < 0.  `spectrum_rest` = the eigenvalues of Q NOT represented in
+    V (all modes outside the l projected ones).  For nu_k > 0 the complement of range((P_+)_exact) carries those plus
+    the projected NEGATIVE eigenvalues (approximated by the negative nu_j), and vice versa."""
+    nu = np.asarray(nu, dtype=np.float64)
+    rest = np.asarray(spectrum_rest, dtype=np.float64)
+    d = np.empty_like(nu)
+    for k, v in enumerate(nu):
+        other = nu[nu < 0] if v > 0 else nu[nu > 0]
+        cand = np.concatenate([rest, other])
+        d[k] = np.min(np.abs(cand - v))
+    return d
+
+
+def kappa_pm(nu, rho, d):
+    """kappa_+-^2 = sum_{+-nu_k > 0} rho_k^2 / d_k^2 (eq. 2.9, PAPER.md:L92).  Returns (kappa_+, kappa_-)."""
+    nu, rho, d = (np.asarray(a, dtype=np.float64) for a in (nu, rho, d))
+    kp = np.sqrt(np.sum((rho[nu > 0] / d[nu > 0]) ** 2))
+    km = np.sqrt(np.sum((rho[nu < 0] / d[nu < 0]) ** 2))
+    return float(kp), float(km)
+
+
+def projector_bound(kappa):
+    """|| P_+- - (P_+-)_exact || <= kappa (1 + 2 kappa) / (1 - 2 kappa (1 + 2 kappa)) (eq. 2.10, PAPER.md:L105);
+    +inf when the denominator is not positive (the bound says nothing there)."""
+    x = 2.0 * kappa * (1.0 + 2.0 * kappa)
+    return float(kappa * (1.0 + 2.0 * kappa) / (1.0 - x)) if x < 1.0 else float("inf")

@@ -48,8 +48,9 @@ SIGNATURES = {
     "nd_set_lowmodes": (_c_int, [_c_vp, _c_int, _c_vp, _pd]),
     "nd_apply_sign": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_int]),
     "nd_apply_DN": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_vp, _c_int]),
-    "nd_lowmodes_compute": (_c_int, [_c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_ull, _c_vp, _pd, _pd,
+    "nd_lowmodes_compute": (_c_int, [_c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_ull, _c_vp, _pd, _pd, _pd,
                                      _c_vp, ctypes.POINTER(_c_ll)]),
+    "nd_projector_error": (_c_int, [_c_int, _pd, _pd, _c_int, _pd, _pd, _pd, _pd]),
     "nd_heev": (_c_int, [_c_int, _pd, _pd, _pd]),
     "nd_axpy": (_c_int, [_c_vp, _pd, _c_vp, _c_vp]),
     "nd_scale": (_c_int, [_c_vp, _pd, _c_vp]),
@@ -115,6 +116,21 @@ def heev(a):
     if rc != ND_OK:
         raise NDError(rc, "nd_heev")
     return w, z
+
+
+def projector_error(nu, rho, rest):
+    """nd_projector_error: (kappa[2], bound[2], d[l]) of eq. 2.9-2.10 - host utility, needs no GPU."""
+    lib = load_library()
+    nu = np.ascontiguousarray(nu, dtype=np.float64)
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    rest = np.ascontiguousarray(rest, dtype=np.float64)
+    kappa, bound, d = np.zeros(2), np.zeros(2), np.zeros(len(nu))
+    rc = lib.nd_projector_error(len(nu), nu.ctypes.data_as(_pd), rho.ctypes.data_as(_pd), len(rest),
+                                rest.ctypes.data_as(_pd) if len(rest) else None, kappa.ctypes.data_as(_pd),
+                                bound.ctypes.data_as(_pd), d.ctypes.data_as(_pd))
+    if rc != ND_OK:
+        raise NDError(rc, "nd_projector_error")
+    return kappa, bound, d
 
 
 def _ptr(x):
@@ -286,12 +302,14 @@ class Context:
         nu = np.zeros(l)
         resid = np.zeros(l)
         stats = (_c_ll * 2)()
+        rest = np.zeros(max(int(lextra), 1))
         rc = self.lib.nd_lowmodes_compute(self._h, int(l), int(lextra), int(degree), float(m), float(tol), int(maxit),
                                           int(seed), u.data_ptr(), nu.ctypes.data_as(_pd), resid.ctypes.data_as(_pd),
-                                          work.data_ptr(), stats)
+                                          rest.ctypes.data_as(_pd), work.data_ptr(), stats)
         if rc not in (ND_OK, -6):
             self._chk(rc)
-        return u, nu, resid, dict(iterations=int(stats[0]), stencils=int(stats[1]), converged=(rc == ND_OK))
+        return u, nu, resid, dict(iterations=int(stats[0]), stencils=int(stats[1]), converged=(rc == ND_OK),
+                                  theta_rest=rest[:int(lextra)])
 
     # -- BLAS-1
     def axpy(self, a, x, y):

@@ -106,8 +106,9 @@ __global__ void compress_gauge_kernel(typename LinkLayout<T, RECON>::LVec* __res
         r[0] = (T)U[0][1].re; r[1] = (T)U[0][1].im;
         r[2] = (T)U[0][2].re; r[3] = (T)U[0][2].im;
         r[4] = (T)U[1][0].re; r[5] = (T)U[1][0].im;
-        r[6] = (T)atan2(U[0][0].im, U[0][0].re);
-        r[7] = (T)atan2(U[2][0].im, U[2][0].re);
+        // the two phases are stored as tan(theta/4) in [-1, 1]: rebuilt with one reciprocal, no sincos (nd_su3.cuh)
+        r[6] = (T)tan(0.25 * atan2(U[0][0].im, U[0][0].re));
+        r[7] = (T)tan(0.25 * atan2(U[2][0].im, U[2][0].re));
     }
     if (!valid) return;
     typename LL::LVec* dst = g + (long long)mu * LL::NL * V + s;

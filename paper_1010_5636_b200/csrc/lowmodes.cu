@@ -94,6 +94,28 @@ extern "C" int nd_heev(int k, const double* a_in, double* w, double* z_out) {
     return ND_OK;
 }
 
+extern "C" int nd_projector_error(int l, const double* nu, const double* rho, int nrest, const double* rest,
+                                  double kappa[2], double bound[2], double* d) {
+    if (l < 1 || !nu || !rho || nrest < 0 || (nrest > 0 && !rest) || !kappa || !bound) return ND_ERR_BAD_ARG;
+    double k2[2] = {0.0, 0.0};
+    for (int k = 0; k < l; k++) {
+        if (nu[k] == 0.0) return ND_ERR_BAD_ARG;   // the sign of nu_k must be unambiguous
+        double dk = INFINITY;
+        for (int j = 0; j < nrest; j++) dk = std::min(dk, std::fabs(rest[j] - nu[k]));
+        for (int j = 0; j < l; j++)
+            if ((nu[j] > 0.0) != (nu[k] > 0.0)) dk = std::min(dk, std::fabs(nu[j] - nu[k]));
+        if (d) d[k] = dk;
+        const double q = rho[k] / dk;
+        k2[nu[k] > 0.0 ? 0 : 1] += q * q;
+    }
+    for (int i = 0; i < 2; i++) {
+        kappa[i] = std::sqrt(k2[i]);
+        const double x = 2.0 * kappa[i] * (1.0 + 2.0 * kappa[i]);
+        bound[i] = (x < 1.0) ? kappa[i] * (1.0 + 2.0 * kappa[i]) / (1.0 - x) : INFINITY;
+    }
+    return ND_OK;
+}
+
 namespace {
 
 struct Solver {
@@ -205,8 +227,8 @@ struct Solver {
 }  // namespace
 
 extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, double m, double tol, int maxit,
-                                   unsigned long long seed, void* u_out, double* nu, double* resid, void* work,
-                                   long long* stats) {
+                                   unsigned long long seed, void* u_out, double* nu, double* resid, double* theta_rest,
+                                   void* work, long long* stats) {
     if (!ctx) return ND_ERR_BAD_ARG;
     if (l < 1 || lextra < 0 || l + lextra > ND_MAX_BLOCK_L || degree < 2 || maxit < 1 || !(tol > 0.0) || !u_out || !nu ||
         !resid || !work)
@@ -281,6 +303,8 @@ extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, d
         if (lextra == 0) cut = std::min(theta[k - 1] * 1.05 + 1e-3, 0.5 * hi);
     }
     if (it > maxit) it = maxit;
+    if (theta_rest)
+        for (int j = l; j < k; j++) theta_rest[j - l] = theta[j];
     // Rayleigh-Ritz of Q in the span of the l lowest vectors (eq. 2.7): Y_j = Q X_j, M = X^dagger Y
     for (int j = 0; j < l; j++) {
         rc = S.Q(S.y(j), S.x(j));

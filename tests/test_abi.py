@@ -115,3 +115,28 @@ def test_product_never_imports_the_oracle():
         if f.endswith((".py", ".c")):
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_1010_5636_b200" not in text.replace("`paper_1010_5636_b200/`", ""), f
+
+
+def test_projector_error_matches_oracle():
+    """nd_projector_error (library, eq. 2.9-2.10) vs the oracle's independent functions on random inputs, and the
+    hand-evaluated value of eq. 2.10 at kappa = 0.1."""
+    import paper_1010_5636_b200 as nd
+    from oracle import lowmodes as olow
+
+    rng = np.random.default_rng(9)
+    for l, nrest in ((1, 0), (6, 5), (20, 12)):
+        nu = rng.uniform(0.3, 0.6, l) * rng.choice([-1.0, 1.0], l)
+        rho = rng.uniform(1e-4, 2e-2, l)
+        rest = rng.uniform(0.7, 1.5, nrest) * rng.choice([-1.0, 1.0], nrest)
+        if l == 1:
+            rest = np.array([0.9])
+        kappa, bound, d = nd.projector_error(nu, rho, rest)
+        dref = olow.distances_d(nu, rest)
+        kp, km = olow.kappa_pm(nu, rho, dref)
+        assert np.allclose(d, dref, rtol=1e-14) and abs(kappa[0] - kp) <= 1e-14 and abs(kappa[1] - km) <= 1e-14
+        for i, k in enumerate((kp, km)):
+            ref = olow.projector_bound(k)
+            assert (np.isinf(ref) and np.isinf(bound[i])) or abs(bound[i] - ref) <= 1e-13 * max(1.0, ref)
+    kappa, bound, _ = nd.projector_error([1.0], [0.1], [2.0])
+    assert abs(kappa[0] - 0.1) < 1e-16 and abs(bound[0] - 0.12 / 0.76) < 1e-15 and kappa[1] == 0 and bound[1] == 0
+    assert np.isinf(nd.projector_error([1.0], [0.5], [2.0])[1][0])

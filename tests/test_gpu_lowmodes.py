@@ -88,3 +88,32 @@ def test_not_converged_is_reported_not_hidden():
     assert not st["converged"] and np.all(np.isfinite(nu)) and np.all(resid > 0)
     with pytest.raises(nd.NDError):
         ctx.lowmodes_compute(300, M)
+
+
+def test_error_control_on_4x4(dense_4x4_smooth):
+    """f1: kappa_+- and the bound (2.10) from the solver's own outputs (nu_k, rho_k, guard Ritz
+    values) against the EXACT projector deviation from the dense eigendecomposition."""
+    import paper_1010_5636_b200 as nd
+
+    d = dense_4x4_smooth
+    ctx, U = make_context(d["dims"], 64, 12, -1, "smooth", eps=0.3)
+    l = 8
+    u, nu, resid, st = ctx.lowmodes_compute(l, M, tol=1e-9, maxit=80, lextra=8, degree=30)
+    assert st["converged"]
+    th = st["theta_rest"]
+    assert len(th) == 8 and np.all(np.diff(th) >= 0) and th[0] >= (nu ** 2).max() - 1e-9
+    lam, W = d["lam"], d["W"]
+    order = np.argsort(lam * lam)
+    assert th[0] >= lam[order[l]] ** 2 - 1e-9          # Ritz values of the guard vectors bound the next eigenvalue from above
+    rest = np.concatenate([np.sqrt(th), -np.sqrt(th)])  # the sign of the next modes of Q is not known: both candidates
+    kappa, bound, dk = nd.projector_error(nu, resid, rest)
+    assert np.all(dk > 0) and np.all(kappa >= 0)
+    Um = np.stack([ctx.unpack_spinor(u[k]).ravel() for k in range(l)], axis=1)
+    low = order[:l]
+    for sgn, i in ((1, 0), (-1, 1)):
+        E = W[:, low[sgn * lam[low] > 0]]
+        A = Um[:, sgn * nu > 0]
+        assert A.shape[1] == E.shape[1]                 # P_+ / P_- split identified without ambiguity (PAPER.md:L81)
+        sv = np.linalg.svd(E.conj().T @ A, compute_uv=False)
+        dev = np.sqrt(max(0.0, 1.0 - sv.min() ** 2))
+        assert dev <= bound[i] + 1e-7, (dev, bound[i], kappa[i])
