@@ -128,6 +128,18 @@ ND_API int nd_set_lowmodes(nd_ctx* ctx, int l, const void* u_soa, const double* 
 ND_API int nd_apply_sign(nd_ctx* ctx, void* out, const void* in, void* work, int use_graph);
 ND_API int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor, void* work, int use_graph);
 
+/* ------------------------------------------------------------------------------- massive operator and solver
+ * nd_apply_DNm: the massive Neuberger-Dirac operator behind the bound (2.12) (R16)
+ *     out = D_N^m in,   D_N^m = (1 - m/(2 prefactor)) D_N + m = (prefactor + m/2) in + (prefactor - m/2) gamma5 sign(Q) in
+ * with prefactor = 1/abar as in nd_apply_DN; one sign-function application.  work: 3 device spinors.
+ * nd_solve_DNm: x = (D_N^m)^{-1} b by conjugate gradients on the normal equations D^dagger D x = D^dagger b,
+ * D^dagger = gamma5 D gamma5; x starts from 0; stops when |D^dagger(b - D x)| <= tol |D^dagger b| or after maxit
+ * iterations (ND_ERR_NO_CONVERGENCE, x still the best iterate).  *relres = |b - D x| / |b| recomputed at the end,
+ * *iters = CG iterations (2 operator applications each).  work: 8 device spinors.  Synchronises (host step lengths). */
+ND_API int nd_apply_DNm(nd_ctx* ctx, void* out, const void* in, double prefactor, double mq, void* work, int use_graph);
+ND_API int nd_solve_DNm(nd_ctx* ctx, void* x, const void* b, double prefactor, double mq, double tol, int maxit, void* work,
+                        double* relres, int* iters);
+
 /* --------------------------------------------------------------------------------------------- low modes
  * The l lowest eigenpairs of Q^2 followed by the Rayleigh-Ritz step of Q in their span
  * (PAPER.md:L81): on return u_out holds u_k (device SoA, l vectors), nu[k] the Ritz values of Q (ascending in

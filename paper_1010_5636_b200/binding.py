@@ -48,6 +48,8 @@ SIGNATURES = {
     "nd_set_lowmodes": (_c_int, [_c_vp, _c_int, _c_vp, _pd]),
     "nd_apply_sign": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_int]),
     "nd_apply_DN": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_vp, _c_int]),
+    "nd_apply_DNm": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_vp, _c_int]),
+    "nd_solve_DNm": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_dbl, _c_int, _c_vp, _pd, ctypes.POINTER(_c_int)]),
     "nd_lowmodes_compute": (_c_int, [_c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_ull, _c_vp, _pd, _pd, _pd,
                                      _c_vp, ctypes.POINTER(_c_ll)]),
     "nd_projector_error": (_c_int, [_c_int, _pd, _pd, _c_int, _pd, _pd, _pd, _pd]),
@@ -294,6 +296,23 @@ class Context:
         assert work.is_contiguous() and work.numel() >= 3 * 24 * self.V
         self._chk(self.lib.nd_apply_DN(self._h, out.data_ptr(), inp.data_ptr(), float(prefactor), work.data_ptr(),
                                        int(use_graph)))
+
+    def apply_DNm(self, out, inp, prefactor, mq, work, use_graph=False):
+        assert work.is_contiguous() and work.numel() >= 3 * 24 * self.V
+        self._chk(self.lib.nd_apply_DNm(self._h, out.data_ptr(), inp.data_ptr(), float(prefactor), float(mq),
+                                        work.data_ptr(), int(use_graph)))
+
+    def solve_DNm(self, x, b, prefactor, mq, tol=1e-8, maxit=500, work=None):
+        """-> (relres, iters, converged); x is overwritten with the solution."""
+        if work is None:
+            work = self.new_spinor(8)
+        assert work.is_contiguous() and work.numel() >= 8 * 24 * self.V
+        relres, iters = ctypes.c_double(), ctypes.c_int()
+        rc = self.lib.nd_solve_DNm(self._h, x.data_ptr(), b.data_ptr(), float(prefactor), float(mq), float(tol), int(maxit),
+                                   work.data_ptr(), ctypes.byref(relres), ctypes.byref(iters))
+        if rc not in (ND_OK, -6):
+            self._chk(rc)
+        return relres.value, iters.value, rc == ND_OK
 
     def lowmodes_compute(self, l, m, tol=1e-8, maxit=50, lextra=8, degree=40, seed=7):
         """-> (u [l, 24V] device tensor, nu[l], resid[l], stats dict)."""

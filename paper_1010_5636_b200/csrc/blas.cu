@@ -147,11 +147,12 @@ __global__ void reduce_partials_kernel(double* __restrict__ out, const double* _
 
 // ------------------------------------------------------------------------------------------- block axpy
 // MODE 0: y <- y + sum_k a_k v_k
-// MODE 1: y <- pref * ( eta + gamma5 ( y + sum_k a_k v_k ) )      (D_N assembly, eq. 2.4 + 2.11)
+// MODE 1: y <- pa * eta + pb * gamma5 ( y + sum_k a_k v_k )       (D_N assembly, eq. 2.4 + 2.11: pa = pb = 1/abar;
+//                                                                   massive operator: pa = 1/abar + m/2, pb = 1/abar - m/2)
 template <typename T, int MODE>
 __global__ void __launch_bounds__(RED_THREADS) block_axpy_kernel(typename Prec<T>::Vec* y, int l, const double* __restrict__ coef,
                                                                  const typename Prec<T>::Vec* __restrict__ v,
-                                                                 const typename Prec<T>::Vec* eta, T pref, long long V) {
+                                                                 const typename Prec<T>::Vec* eta, T pa, T pb, long long V) {
     extern __shared__ double sm[];   // [2l]
     for (int i = threadIdx.x; i < 2 * l; i += blockDim.x) sm[i] = coef[i];
     __syncthreads();
@@ -171,7 +172,7 @@ __global__ void __launch_bounds__(RED_THREADS) block_axpy_kernel(typename Prec<T
 #pragma unroll
             for (int i = 0; i < 12; i++) {
                 const T sg = (i < 6) ? T(1) : T(-1);
-                c[i] = {pref * (e[i].re + sg * c[i].re), pref * (e[i].im + sg * c[i].im)};
+                c[i] = {fma(pa, e[i].re, pb * sg * c[i].re), fma(pa, e[i].im, pb * sg * c[i].im)};
             }
         }
         store_site<T>(y, V, s, c);
@@ -262,17 +263,18 @@ int ndi_block_dot2_dev(nd_ctx* ctx, int l, const void* v, const void* x0, const 
     return (ctx->prec == 32) ? block_dot_t<float>(ctx, l, 2, v, x0, x1, d_out) : block_dot_t<double>(ctx, l, 2, v, x0, x1, d_out);
 }
 // y <- y + sum_k coef_k v_k (mode 0) or the D_N assembly (mode 1); coef on the device
-int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pref) {
+int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pa,
+                       double pb) {
     const unsigned blocks = grid_for(ctx->V, RED_THREADS, 1 << 30);
     const size_t smem = (size_t)2 * (l > 0 ? l : 1) * sizeof(double);
     if (ctx->prec == 32) {
         using Vec = float4;
-        if (mode == 0) block_axpy_kernel<float, 0><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, nullptr, 0.f, ctx->V);
-        else block_axpy_kernel<float, 1><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, (const Vec*)eta, (float)pref, ctx->V);
+        if (mode == 0) block_axpy_kernel<float, 0><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, nullptr, 0.f, 0.f, ctx->V);
+        else block_axpy_kernel<float, 1><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, (const Vec*)eta, (float)pa, (float)pb, ctx->V);
     } else {
         using Vec = double2;
-        if (mode == 0) block_axpy_kernel<double, 0><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, nullptr, 0.0, ctx->V);
-        else block_axpy_kernel<double, 1><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, (const Vec*)eta, pref, ctx->V);
+        if (mode == 0) block_axpy_kernel<double, 0><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, nullptr, 0.0, 0.0, ctx->V);
+        else block_axpy_kernel<double, 1><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, (const Vec*)eta, pa, pb, ctx->V);
     }
     ND_LAUNCHED(ctx);
     return ND_OK;
@@ -337,7 +339,7 @@ extern "C" int nd_block_axpy(nd_ctx* ctx, int l, const double* a2l, const void* 
     ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int i = 0; i < 2 * l; i++) ctx->h_result[i] = a2l[i];
     ND_CUDA(ctx, cudaMemcpyAsync(ctx->d_coef, ctx->h_result, (size_t)2 * l * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    return ndi_block_axpy_dev(ctx, l, ctx->d_coef, v, y, 0, nullptr, 0.0);
+    return ndi_block_axpy_dev(ctx, l, ctx->d_coef, v, y, 0, nullptr, 0.0, 0.0);
 }
 extern "C" int nd_gaussian(nd_ctx* ctx, void* x, unsigned long long seed) {
     ND_ENTER(ctx);

@@ -168,7 +168,7 @@ struct Solver {
         ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));   // `col` is pageable and dies with this frame
         ND_CUDA(ctx, cudaMemsetAsync(dst, 0, (size_t)nd * sb, ctx->stream));
         for (int j = 0; j < nd; j++) {
-            int rc = ndi_block_axpy_dev(ctx, ns, d_mat + (size_t)2 * ns * j, src, dst + (size_t)j * sb, 0, nullptr, 0.0);
+            int rc = ndi_block_axpy_dev(ctx, ns, d_mat + (size_t)2 * ns * j, src, dst + (size_t)j * sb, 0, nullptr, 0.0, 0.0);
             if (rc != ND_OK) return rc;
         }
         return ND_OK;

@@ -21,8 +21,8 @@ struct nd_graph_entry {
     void* out;
     const void* in;
     void* work;
-    int kind;            // 0 sign, 1 D_N
-    double prefactor;
+    int kind;            // 0 sign, 1 D_N / D_N^m
+    double pa, pb;       // out = pa*in + pb*gamma5 sign(Q) in
     cudaGraphExec_t exec;
     long long nodes;     // kernel launches one replay stands for
 };
@@ -148,7 +148,9 @@ int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, doub
                 double s2, const void* v2, double s3, const void* v3);
 int ndi_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out);   // d_out: 2l doubles (device)
 int ndi_block_dot2_dev(nd_ctx* ctx, int l, const void* v, const void* x0, const void* x1, double* d_out);  // 4l doubles
-int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pref);
+int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pa,
+                       double pb);   // mode 1: y <- pa*eta + pb*gamma5(y + sum_k a_k v_k)
+int ndi_apply_DNm(nd_ctx* ctx, void* out, const void* in, double pa, double pb, void* work, int use_graph);
 int ndi_read_result(nd_ctx* ctx, const double* d_src, double* h_dst, int n);              // sync copy to host
 int ndi_drop_graphs(nd_ctx* ctx);
 constexpr int ND_RESULT_DOUBLES = 4 * ND_MAX_BLOCK_L;

@@ -47,7 +47,7 @@ int scale_copy(nd_ctx* ctx, void* y, const void* x, double a) {
 }
 
 // kind 0: out = sign(Q) in ; kind 1: out = prefactor (in + gamma5 sign(Q) in)
-int enqueue_sign(nd_ctx* ctx, void* out, const void* eta, void* work, int kind, double prefactor) {
+int enqueue_sign(nd_ctx* ctx, void* out, const void* eta, void* work, int kind, double pa, double pb) {
     const size_t sb = nd_spinor_bytes(ctx);
     char* bA = (char*)work;
     char* bB = bA + sb;
@@ -86,28 +86,28 @@ int enqueue_sign(nd_ctx* ctx, void* out, const void* eta, void* work, int kind, 
         ND_LAUNCHED(ctx);
     }
     if (l > 0 || kind == 1) {
-        rc = ndi_block_axpy_dev(ctx, l, ctx->d_coef, ctx->u, out, kind, eta, prefactor);
+        rc = ndi_block_axpy_dev(ctx, l, ctx->d_coef, ctx->u, out, kind, eta, pa, pb);
         if (rc != ND_OK) return rc;
     }
     return ND_OK;
 }
 
-int apply_sign_impl(nd_ctx* ctx, void* out, const void* in, void* work, int kind, double prefactor, int use_graph) {
+int apply_sign_impl(nd_ctx* ctx, void* out, const void* in, void* work, int kind, double pa, double pb, int use_graph) {
     if (!ctx) return ND_ERR_BAD_ARG;
     if (!out || !in || !work || out == in) return nd_fail(ctx, ND_ERR_BAD_ARG, "apply_sign/DN: null or aliased argument");
     if (!ctx->gauge_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_sign/DN: gauge field not set");
     if (!ctx->poly_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_sign/DN: polynomial not set (nd_set_sign_poly)");
     ND_CUDA(ctx, cudaSetDevice(ctx->device));
-    if (!use_graph || ctx->stream == nullptr) return enqueue_sign(ctx, out, in, work, kind, prefactor);
+    if (!use_graph || ctx->stream == nullptr) return enqueue_sign(ctx, out, in, work, kind, pa, pb);
     for (auto& g : ctx->graphs)
-        if (g.out == out && g.in == in && g.work == work && g.kind == kind && g.prefactor == prefactor) {
+        if (g.out == out && g.in == in && g.work == work && g.kind == kind && g.pa == pa && g.pb == pb) {
             ND_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
             ctx->launches += g.nodes;
             return ND_OK;
         }
     const long long before = ctx->launches;
     ND_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
-    int rc = enqueue_sign(ctx, out, in, work, kind, prefactor);
+    int rc = enqueue_sign(ctx, out, in, work, kind, pa, pb);
     cudaGraph_t graph = nullptr;
     cudaError_t e = cudaStreamEndCapture(ctx->stream, &graph);
     const long long nodes = ctx->launches - before;
@@ -118,7 +118,7 @@ int apply_sign_impl(nd_ctx* ctx, void* out, const void* in, void* work, int kind
     }
     ND_CUDA(ctx, e);
     nd_graph_entry g;
-    g.out = out; g.in = in; g.work = work; g.kind = kind; g.prefactor = prefactor; g.exec = nullptr; g.nodes = nodes;
+    g.out = out; g.in = in; g.work = work; g.kind = kind; g.pa = pa; g.pb = pb; g.exec = nullptr; g.nodes = nodes;
     e = cudaGraphInstantiate(&g.exec, graph, 0);
     cudaGraphDestroy(graph);
     ND_CUDA(ctx, e);
@@ -130,6 +130,10 @@ int apply_sign_impl(nd_ctx* ctx, void* out, const void* in, void* work, int kind
 }
 
 }  // namespace
+
+int ndi_apply_DNm(nd_ctx* ctx, void* out, const void* in, double pa, double pb, void* work, int use_graph) {
+    return apply_sign_impl(ctx, out, in, work, 1, pa, pb, use_graph);
+}
 
 // --------------------------------------------------------------------------------------------------- C ABI
 extern "C" int nd_cheb_coeffs(int n, double eps, double* c, double* delta) {
@@ -206,8 +210,8 @@ extern "C" int nd_set_lowmodes(nd_ctx* ctx, int l, const void* u_soa, const doub
 }
 
 extern "C" int nd_apply_sign(nd_ctx* ctx, void* out, const void* in, void* work, int use_graph) {
-    return apply_sign_impl(ctx, out, in, work, 0, 0.0, use_graph);
+    return apply_sign_impl(ctx, out, in, work, 0, 0.0, 0.0, use_graph);
 }
 extern "C" int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor, void* work, int use_graph) {
-    return apply_sign_impl(ctx, out, in, work, 1, prefactor, use_graph);
+    return apply_sign_impl(ctx, out, in, work, 1, prefactor, prefactor, use_graph);
 }

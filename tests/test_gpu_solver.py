@@ -1,0 +1,74 @@
+"""the massive operator D_N^m (R16) and its CG inversion on the CUDA path against the oracle's
+operator and textbook CG with the same polynomial coefficients."""
+import numpy as np
+import pytest
+
+from lattice_inputs import gaussian_spinor
+from oracle import sign as osign
+from oracle import solver as osolver
+from oracle import wilson, wilson_c
+from tests.gpu_common import make_context, rel_l2, round_to
+
+pytestmark = pytest.mark.gpu
+
+RHO = 1.6
+M = -RHO
+QNORM = 6.4
+
+
+def setup(prec, dims=(8, 4, 4, 8), n=60, eps=0.004):
+    ctx, U = make_context(dims, prec, 12, -1, "smooth", eps=0.3)
+    c = osign.cheb_coeffs(n, eps)
+    ctx.set_sign_poly(c, eps, QNORM, M)
+    ctx.set_lowmodes(None, [])
+    Q = wilson_c.make_Q(U, M, -1)
+    DN = lambda v: osign.apply_DN(Q, wilson.apply_gamma5, v, c, eps, QNORM, RHO)     # prefactor 1/abar = rho
+    return ctx, DN
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("mq", [0.0, 0.1, 0.5])
+def test_apply_DNm(prec, mq):
+    ctx, DN = setup(prec)
+    eta = round_to(gaussian_spinor(ctx.dims), prec)
+    out, work = ctx.new_spinor(), ctx.new_spinor(3)
+    ctx.apply_DNm(out, ctx.pack_spinor(eta), RHO, mq, work, use_graph=True)
+    ref = osolver.apply_DNm(DN, eta, 1.0 / RHO, mq)
+    assert rel_l2(ctx.unpack_spinor(out), ref) <= (1e-11 if prec == 64 else 1e-5)
+
+
+def test_solve_fp64_matches_oracle_cg():
+    ctx, DN = setup(64)
+    mq, tol = 0.2, 1e-9
+    b = gaussian_spinor(ctx.dims)
+    x = ctx.new_spinor()
+    relres, iters, ok = ctx.solve_DNm(x, ctx.pack_spinor(b), RHO, mq, tol=tol, maxit=300)
+    assert ok and relres < 1e-7
+    D = lambda v: osolver.apply_DNm(DN, v, 1.0 / RHO, mq)
+    Dd = lambda v: wilson.apply_gamma5(D(wilson.apply_gamma5(v)))
+    xr, itr, resr = osolver.cg_normal_equations(D, Dd, b, tol, 300)
+    got = ctx.unpack_spinor(x)
+    assert abs(iters - itr) <= 2
+    assert rel_l2(got, xr) <= 1e-7
+    assert np.linalg.norm((b - D(got)).ravel()) <= 1e-7 * np.linalg.norm(b.ravel())     # the oracle's operator agrees
+
+
+def test_solve_fp32_and_failure_reporting():
+    import paper_1010_5636_b200 as nd
+
+    ctx, DN = setup(32)
+    mq = 0.3
+    b = round_to(gaussian_spinor(ctx.dims), 32)
+    x, bd = ctx.new_spinor(), ctx.pack_spinor(b)
+    relres, iters, ok = ctx.solve_DNm(x, bd, RHO, mq, tol=1e-4, maxit=200)
+    assert ok and relres < 1e-3
+    D = lambda v: osolver.apply_DNm(DN, v, 1.0 / RHO, mq)
+    assert np.linalg.norm((b - D(ctx.unpack_spinor(x))).ravel()) <= 2e-3 * np.linalg.norm(b.ravel())
+    relres2, iters2, ok2 = ctx.solve_DNm(x, bd, RHO, mq, tol=1e-12, maxit=2)     # cannot converge in 2 iterations
+    assert not ok2 and iters2 == 2 and 0 < relres2 < 1
+    with pytest.raises(nd.NDError):
+        ctx.solve_DNm(bd, bd, RHO, mq)                                            # aliasing
+    # zero right-hand side
+    z = ctx.new_spinor()
+    z.zero_()
+    assert ctx.solve_DNm(x, z, RHO, mq) == (0.0, 0, True)
