@@ -51,6 +51,8 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->u = nullptr;
     ctx->launches = 0;
     ctx->capturing = false;
+    ctx->num_sms = 148;
+    cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     ctx->err[0] = 0;
     // fp32 recon 18 is stored as 9 float2, everything else in 128-bit words: bytes = 4 * recon * V * prec/8
     ctx->gauge_bytes = (size_t)4 * recon * ctx->V * (prec / 8);

@@ -55,6 +55,7 @@ struct nd_ctx {
     std::vector<nd_graph_entry> graphs;
     long long launches;
     bool capturing;
+    int num_sms;
     char err[512];
 };
 

@@ -222,7 +222,9 @@ int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double 
     G.S1 = (long long)G.L2 * G.L3;
     G.S0 = (long long)G.L1 * G.L2 * G.L3;
     G.bc = ctx->bc;
-    const int threads = 128;
+    // 128 threads per CTA; small lattices (launch-latency-bound, BASELINE config 3) get smaller CTAs so that every SM has work
+    int threads = 128;
+    while (threads > 32 && ctx->V / threads < 2 * ctx->num_sms) threads /= 2;
     const unsigned blocks = (unsigned)((ctx->V + threads - 1) / threads);
     if (epi)
         wilson_Q_kernel<T, RECON, true><<<blocks, threads, 0, ctx->stream>>>(
