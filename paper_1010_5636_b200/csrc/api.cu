@@ -1,5 +1,6 @@
 // api.cu - context life cycle and error reporting of the C-ABI library (include/nd_b200.h).
 #include <cstdarg>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -51,6 +52,28 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->u = nullptr;
     ctx->launches = 0;
     ctx->capturing = false;
+    {
+        // stencil CTA tile (x1, x2, x3) of 128 sites: x3 extent = the largest power of two <= 32 dividing L3, then x2 and
+        // x1 are doubled in turn while they divide the lattice (32^3: 2 x 2 x 32).  ND_TILE="b1,b2,b3" caps the extents
+        // (tuning only), "0" forces the linear mapping; lattices without a tile of >= 64 sites use the linear mapping.
+        int cap[3] = {128, 128, 32};
+        const char* e = getenv("ND_TILE");
+        if (e) sscanf(e, "%d,%d,%d", &cap[0], &cap[1], &cap[2]);
+        int lb[3] = {0, 0, 0}, threads = 1;
+        auto grow = [&](int i) {
+            if (threads * 2 > 128 || (2 << lb[i]) > cap[i] || dims[i + 1] % (2 << lb[i]) != 0) return false;
+            lb[i]++;
+            threads *= 2;
+            return true;
+        };
+        while (grow(2)) {}
+        for (bool g = true; g;) {
+            g = grow(1);
+            g = grow(0) || g;
+        }
+        for (int i = 0; i < 3; i++) ctx->tile_lb[i] = lb[i];
+        ctx->tile_threads = (threads >= 64 && !(e && e[0] == '0' && e[1] == 0)) ? threads : 0;
+    }
     ctx->num_sms = 148;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     ctx->err[0] = 0;

@@ -21,6 +21,9 @@ struct Geom {
     long long S1, S2;   // strides of x1, x0 in sites: S2 = L3 (x2 stride), S1 = L2*L3, S0 = L1*L2*L3
     long long S0;
     int bc;             // +1 / -1
+    // CTA tile in (x1, x2, x3): 2^lb[i] sites along x_{i+1}, nt[i] tiles; nt[2] == 0: linear mapping
+    int lb[3];
+    int nt[3];
 };
 
 template <typename T>
@@ -111,11 +114,11 @@ __device__ __forceinline__ void hop_pair(const typename Prec<T>::Vec* __restrict
     accumulate<T, MU, +1>(g, acc);
 }
 
-// out(x) = gamma5 [ (4+m) phi(x) - 1/2 acc ], optionally followed by the fused vector update
+// out(x) = gamma5 [ -1/2 acc ] (acc holds -2 (4+m) phi(x) + the eight hops), optionally followed by the fused vector update
 // out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3 (every v_i(x) is read before the store, so out may alias them)
 template <typename T, bool EPI>
 __device__ __forceinline__ void finish_site(typename Prec<T>::Vec* __restrict__ out, long long V, long long s,
-                                            const cx<T> (&phi)[12], const cx<T> (&acc)[12], T mass_term, T s0, T s1,
+                                            const cx<T> (&acc)[12], T s0, T s1,
                                             const typename Prec<T>::Vec* v1, T s2, const typename Prec<T>::Vec* v2, T s3,
                                             const typename Prec<T>::Vec* v3) {
     using Vec = typename Prec<T>::Vec;
@@ -123,9 +126,9 @@ __device__ __forceinline__ void finish_site(typename Prec<T>::Vec* __restrict__ 
     cx<T> res[12];
 #pragma unroll
     for (int i = 0; i < 12; i++) {
-        T sg = (i < 6) ? T(1) : T(-1);
-        res[i].re = sg * fma(T(-0.5), acc[i].re, mass_term * phi[i].re);
-        res[i].im = sg * fma(T(-0.5), acc[i].im, mass_term * phi[i].im);
+        const T sg = (i < 6) ? T(-0.5) : T(0.5);
+        res[i].re = sg * acc[i].re;
+        res[i].im = sg * acc[i].im;
     }
     Vec w[NV];
     cx_to_words(res, w);
@@ -153,6 +156,9 @@ __device__ __forceinline__ void finish_site(typename Prec<T>::Vec* __restrict__ 
     for (int p = 0; p < NV; p++) out[p * V + s] = w[p];
 }
 
+#ifndef ND_Q_THREADS
+#define ND_Q_THREADS 128
+#endif
 #ifndef ND_MINB32
 #define ND_MINB32 5
 #endif
@@ -163,31 +169,46 @@ __device__ __forceinline__ void finish_site(typename Prec<T>::Vec* __restrict__ 
 template <typename T> constexpr int q_min_blocks() { return sizeof(T) == 4 ? ND_MINB32 : ND_MINB64; }
 
 template <typename T, int RECON, bool EPI>
-__global__ void __launch_bounds__(128, q_min_blocks<T>()) wilson_Q_kernel(typename Prec<T>::Vec* __restrict__ out,
+__global__ void __launch_bounds__(ND_Q_THREADS, q_min_blocks<T>()) wilson_Q_kernel(typename Prec<T>::Vec* __restrict__ out,
                                                        const typename Prec<T>::Vec* __restrict__ in,
                                                        const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, Geom G,
                                                        T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2,
                                                        const typename Prec<T>::Vec* v2, T s3,
                                                        const typename Prec<T>::Vec* v3) {
-    long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= G.V) return;
-    int x3 = (int)(s % G.L3);
-    long long r = s / G.L3;
-    int x2 = (int)(r % G.L2);
-    r /= G.L2;
-    int x1 = (int)(r % G.L1);
-    int x0 = (int)(r / G.L1);
+    long long s;
+    int x0, x1, x2, x3;
+    if (G.nt[2] == 0) {
+        s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        if (s >= G.V) return;
+        x3 = (int)(s % G.L3);
+        long long r = s / G.L3;
+        x2 = (int)(r % G.L2);
+        r /= G.L2;
+        x1 = (int)(r % G.L1);
+        x0 = (int)(r / G.L1);
+    } else {
+        // the CTA covers a (x1, x2, x3) block of one time-slice: its x1/x2/x3 neighbours are re-read through L1
+        unsigned t = threadIdx.x, b = blockIdx.x;
+        x3 = (int)(t & ((1u << G.lb[2]) - 1)); t >>= G.lb[2];
+        x2 = (int)(t & ((1u << G.lb[1]) - 1)); t >>= G.lb[1];
+        x1 = (int)t;
+        x3 += (int)(b % G.nt[2]) << G.lb[2]; b /= G.nt[2];
+        x2 += (int)(b % G.nt[1]) << G.lb[1]; b /= G.nt[1];
+        x1 += (int)(b % G.nt[0]) << G.lb[0]; b /= G.nt[0];
+        x0 = (int)b;
+        s = (((long long)x0 * G.L1 + x1) * G.L2 + x2) * G.L3 + x3;
+    }
 
+    // The centre and the x1/x2/x3 hops come first: those are the lines neighbouring threads of the CTA share, and the
+    // sooner after one another they are requested the more of them L1 still holds.  The time hops (no reuse inside the
+    // CTA) come last.  The mass term enters through the accumulator: -1/2 acc = (4+m) phi - 1/2 sum(hops).
     cx<T> acc[12];
-#pragma unroll
-    for (int i = 0; i < 12; i++) acc[i] = {T(0), T(0)};
-
     {
-        long long sf = (x0 == G.L0 - 1) ? s - (long long)(G.L0 - 1) * G.S0 : s + G.S0;
-        long long sb = (x0 == 0) ? s + (long long)(G.L0 - 1) * G.S0 : s - G.S0;
-        T pf = (x0 == G.L0 - 1) ? T(G.bc) : T(1);
-        T pb = (x0 == 0) ? T(G.bc) : T(1);
-        hop_pair<T, RECON, 0>(in, gauge, G, s, sf, sb, pf, pb, acc);
+        cx<T> phi[12];
+        load_spinor<T>(in, G.V, s, phi);
+        const T f = T(-2) * mass_term;
+#pragma unroll
+        for (int i = 0; i < 12; i++) acc[i] = {f * phi[i].re, f * phi[i].im};
     }
     {
         long long sf = (x1 == G.L1 - 1) ? s - (long long)(G.L1 - 1) * G.S1 : s + G.S1;
@@ -204,10 +225,15 @@ __global__ void __launch_bounds__(128, q_min_blocks<T>()) wilson_Q_kernel(typena
         long long sb = (x3 == 0) ? s + (G.L3 - 1) : s - 1;
         hop_pair<T, RECON, 3>(in, gauge, G, s, sf, sb, T(1), T(1), acc);
     }
+    {
+        long long sf = (x0 == G.L0 - 1) ? s - (long long)(G.L0 - 1) * G.S0 : s + G.S0;
+        long long sb = (x0 == 0) ? s + (long long)(G.L0 - 1) * G.S0 : s - G.S0;
+        T pf = (x0 == G.L0 - 1) ? T(G.bc) : T(1);
+        T pb = (x0 == 0) ? T(G.bc) : T(1);
+        hop_pair<T, RECON, 0>(in, gauge, G, s, sf, sb, pf, pb, acc);
+    }
 
-    cx<T> phi[12];
-    load_spinor<T>(in, G.V, s, phi);
-    finish_site<T, EPI>(out, G.V, s, phi, acc, mass_term, s0, s1, v1, s2, v2, s3, v3);
+    finish_site<T, EPI>(out, G.V, s, acc, s0, s1, v1, s2, v2, s3, v3);
 }
 
 template <typename T, int RECON>
@@ -225,7 +251,13 @@ int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double 
     // 128 threads per CTA; small lattices (launch-latency-bound, BASELINE config 3) get smaller CTAs so that every SM has work
     int threads = 128;
     while (threads > 32 && ctx->V / threads < 2 * ctx->num_sms) threads /= 2;
-    const unsigned blocks = (unsigned)((ctx->V + threads - 1) / threads);
+    unsigned blocks = (unsigned)((ctx->V + threads - 1) / threads);
+    for (int i = 0; i < 3; i++) { G.lb[i] = ctx->tile_lb[i]; G.nt[i] = 0; }
+    if (ctx->tile_threads > 0 && ctx->tile_threads <= ND_Q_THREADS && ctx->V / ctx->tile_threads >= 2 * ctx->num_sms) {
+        threads = ctx->tile_threads;
+        blocks = (unsigned)G.L0;
+        for (int i = 0; i < 3; i++) { G.nt[i] = ctx->dims[i + 1] >> G.lb[i]; blocks *= (unsigned)G.nt[i]; }
+    }
     if (epi)
         wilson_Q_kernel<T, RECON, true><<<blocks, threads, 0, ctx->stream>>>(
             (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(s0), T(s1), (const Vec*)v1, T(s2),
