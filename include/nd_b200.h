@@ -90,6 +90,9 @@ ND_API int nd_gauge_stats(nd_ctx* ctx, double out[3]);
  * precision.  `soa` is always device memory of nd_spinor_bytes(ctx). */
 ND_API int nd_pack_spinor(nd_ctx* ctx, const void* aos, int aos_prec, int aos_on_device, void* soa);
 ND_API int nd_unpack_spinor(nd_ctx* ctx, const void* soa, void* aos, int aos_prec, int aos_on_device);
+/* Device SoA spinor of precision src_prec -> device SoA spinor of precision dst_prec (32 / 64) on ctx's lattice and stream
+ * (round to nearest when narrowing); the context's own precision does not matter.  dst != src. */
+ND_API int nd_convert_spinor(nd_ctx* ctx, void* dst, int dst_prec, const void* src, int src_prec);
 
 /* --------------------------------------------------------------------------------------------- operators
  * out = Q in,  Q = gamma5 D_W,
@@ -139,6 +142,15 @@ ND_API int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor,
 ND_API int nd_apply_DNm(nd_ctx* ctx, void* out, const void* in, double prefactor, double mq, void* work, int use_graph);
 ND_API int nd_solve_DNm(nd_ctx* ctx, void* x, const void* b, double prefactor, double mq, double tol, int maxit, void* work,
                         double* relres, int* iters);
+/* Mixed precision ("fp32 inner Q applications with fp64 accumulation", BASELINE.json config 4): iterative
+ * refinement x <- x + e, D e = r solved by nd_solve_DNm in the fp32 context ctx32 to inner_tol, r = b - D x recomputed in
+ * the fp64 context ctx64 once per outer step, until |b - D x| <= tol |b|.  Both contexts must describe the same lattice on
+ * the same device and have the same gauge field and polynomial set.  x, b: fp64 device spinors.
+ * work64: 6 fp64 spinors, work32: 10 fp32 spinors.  stats (may be NULL): [0] outer steps (= fp64 operator applications),
+ * [1] fp32 CG iterations in total. */
+ND_API int nd_solve_DNm_mixed(nd_ctx* ctx64, nd_ctx* ctx32, void* x, const void* b, double prefactor, double mq, double tol,
+                              double inner_tol, int max_outer, int max_inner, void* work64, void* work32, double* relres,
+                              int* stats);
 
 /* --------------------------------------------------------------------------------------------- low modes
  * The l lowest eigenpairs of Q^2 followed by the Rayleigh-Ritz step of Q in their span

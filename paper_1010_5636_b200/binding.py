@@ -50,6 +50,9 @@ SIGNATURES = {
     "nd_apply_DN": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_vp, _c_int]),
     "nd_apply_DNm": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_vp, _c_int]),
     "nd_solve_DNm": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_dbl, _c_int, _c_vp, _pd, ctypes.POINTER(_c_int)]),
+    "nd_solve_DNm_mixed": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_dbl, _c_dbl, _c_int, _c_int, _c_vp, _c_vp, _pd,
+                                    ctypes.POINTER(_c_int)]),
+    "nd_convert_spinor": (_c_int, [_c_vp, _c_vp, _c_int, _c_vp, _c_int]),
     "nd_lowmodes_compute": (_c_int, [_c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_ull, _c_vp, _pd, _pd, _pd,
                                      _c_vp, ctypes.POINTER(_c_ll)]),
     "nd_projector_error": (_c_int, [_c_int, _pd, _pd, _c_int, _pd, _pd, _pd, _pd]),
@@ -313,6 +316,22 @@ class Context:
         if rc not in (ND_OK, -6):
             self._chk(rc)
         return relres.value, iters.value, rc == ND_OK
+
+    def solve_DNm_mixed(self, ctx32, x, b, prefactor, mq, tol=1e-10, inner_tol=1e-4, max_outer=20, max_inner=500):
+        """self: the fp64 context; ctx32: an fp32 context of the same lattice -> (relres, outer, inner_iters, converged)."""
+        work64, work32 = self.new_spinor(6), ctx32.new_spinor(10)
+        relres, stats = ctypes.c_double(), (_c_int * 2)()
+        self.synchronize()
+        ctx32.synchronize()
+        rc = self.lib.nd_solve_DNm_mixed(self._h, ctx32._h, x.data_ptr(), b.data_ptr(), float(prefactor), float(mq), float(tol),
+                                         float(inner_tol), int(max_outer), int(max_inner), work64.data_ptr(),
+                                         work32.data_ptr(), ctypes.byref(relres), stats)
+        if rc not in (ND_OK, -6):
+            self._chk(rc)
+        return relres.value, int(stats[0]), int(stats[1]), rc == ND_OK
+
+    def convert_spinor(self, dst, dst_prec, src, src_prec):
+        self._chk(self.lib.nd_convert_spinor(self._h, dst.data_ptr(), int(dst_prec), src.data_ptr(), int(src_prec)))
 
     def lowmodes_compute(self, l, m, tol=1e-8, maxit=50, lextra=8, degree=40, seed=7):
         """-> (u [l, 24V] device tensor, nu[l], resid[l], stats dict)."""

@@ -39,6 +39,25 @@ __global__ void unpack_spinor_kernel(Tout* __restrict__ aos, const typename Prec
     for (int k = 0; k < W; k++) aos[s * 24 + p * W + k] = (Tout)wr[k];
 }
 
+// device SoA of one precision -> device SoA of the other (mixed-precision solver): thread = site
+template <typename Td, typename Ts>
+__global__ void convert_spinor_kernel(typename Prec<Td>::Vec* __restrict__ dst, const typename Prec<Ts>::Vec* __restrict__ src, long long V) {
+    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= V) return;
+    typename Prec<Ts>::Vec ws[Prec<Ts>::NV];
+#pragma unroll
+    for (int p = 0; p < Prec<Ts>::NV; p++) ws[p] = src[p * V + s];
+    cx<Ts> cs[12];
+    words_to_cx(ws, cs);
+    cx<Td> cd[12];
+#pragma unroll
+    for (int i = 0; i < 12; i++) cd[i] = {(Td)cs[i].re, (Td)cs[i].im};
+    typename Prec<Td>::Vec wd[Prec<Td>::NV];
+    cx_to_words(cd, wd);
+#pragma unroll
+    for (int p = 0; p < Prec<Td>::NV; p++) dst[p * V + s] = wd[p];
+}
+
 // --------------------------------------------------------------------------------------------------- links
 __device__ __forceinline__ void atomic_max_nonneg(double* addr, double v) {
     atomicMax(reinterpret_cast<unsigned long long*>(addr), (unsigned long long)__double_as_longlong(v));
@@ -291,4 +310,21 @@ extern "C" int nd_unpack_spinor(nd_ctx* ctx, const void* soa, void* aos, int aos
     }
     if (d_tmp) cudaFreeAsync(d_tmp, ctx->stream);
     return rc;
+}
+
+extern "C" int nd_convert_spinor(nd_ctx* ctx, void* dst, int dst_prec, const void* src, int src_prec) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (!dst || !src || dst == src || (dst_prec != 32 && dst_prec != 64) || (src_prec != 32 && src_prec != 64))
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "convert_spinor: bad argument");
+    ND_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (dst_prec == src_prec) {
+        ND_CUDA(ctx, cudaMemcpyAsync(dst, src, (size_t)24 * ctx->V * (src_prec / 8), cudaMemcpyDeviceToDevice, ctx->stream));
+        return ND_OK;
+    }
+    const int threads = 128;
+    const unsigned blocks = (unsigned)((ctx->V + threads - 1) / threads);
+    if (dst_prec == 32) convert_spinor_kernel<float, double><<<blocks, threads, 0, ctx->stream>>>((float4*)dst, (const double2*)src, ctx->V);
+    else convert_spinor_kernel<double, float><<<blocks, threads, 0, ctx->stream>>>((double2*)dst, (const float4*)src, ctx->V);
+    ND_LAUNCHED(ctx);
+    return ND_OK;
 }

@@ -87,3 +87,57 @@ extern "C" int nd_solve_DNm(nd_ctx* ctx, void* x, const void* b, double prefacto
     if (!ok) return nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "solve_DNm: %d iterations, |D^dagger r|/|D^dagger b| = %.3e > tol %.3e", it, std::sqrt(rr / (stop / (tol * tol))), tol);
     return ND_OK;
 }
+
+// Mixed precision ("fp32-inner / fp64-outer"): iterative refinement.  The fp64 context owns x, b and
+// the residual r = b - D x, recomputed in fp64 once per outer step; the correction D e = r is solved in the fp32 context
+// (same lattice, gauge field and polynomial) to a loose tolerance and added in fp64.
+extern "C" int nd_solve_DNm_mixed(nd_ctx* ctx64, nd_ctx* ctx32, void* x, const void* b, double prefactor, double mq, double tol,
+                                  double inner_tol, int max_outer, int max_inner, void* work64, void* work32, double* relres,
+                                  int* stats) {
+    if (!ctx64 || !ctx32) return ND_ERR_BAD_ARG;
+    if (ctx64->prec != 64 || ctx32->prec != 32 || ctx64->V != ctx32->V || ctx64->device != ctx32->device)
+        return nd_fail(ctx64, ND_ERR_BAD_ARG, "solve_DNm_mixed: needs an fp64 and an fp32 context of the same lattice and device");
+    for (int i = 0; i < 4; i++)
+        if (ctx64->dims[i] != ctx32->dims[i]) return nd_fail(ctx64, ND_ERR_BAD_ARG, "solve_DNm_mixed: lattices differ");
+    if (!x || !b || x == b || !work64 || !work32 || !(tol > 0.0) || !(inner_tol > 0.0) || max_outer < 1 || max_inner < 1)
+        return nd_fail(ctx64, ND_ERR_BAD_ARG, "solve_DNm_mixed: bad argument");
+    const size_t sb64 = nd_spinor_bytes(ctx64), sb32 = nd_spinor_bytes(ctx32);
+    char* w64 = (char*)work64;
+    char* w32 = (char*)work32;
+    void *r = w64, *t = w64 + sb64, *e64 = w64 + 2 * sb64, *sw = w64 + 3 * sb64;   // 6 fp64 spinors
+    void *r32 = w32, *e32 = w32 + sb32, *iw = w32 + 2 * sb32;                      // 2 + 8 fp32 spinors
+    const double pa = prefactor + 0.5 * mq, pb = prefactor - 0.5 * mq;
+    const double one[2] = {1.0, 0.0}, m1[2] = {-1.0, 0.0};
+    int outer = 0, inner_total = 0, rc;
+    double bb = 0.0, rr = 0.0;
+    rc = nd_norm2(ctx64, b, &bb);
+    if (rc != ND_OK) return rc;
+    ND_CUDA(ctx64, cudaMemsetAsync(x, 0, sb64, ctx64->stream));
+    rc = nd_copy(ctx64, r, b);
+    if (rc != ND_OK) return rc;
+    rr = bb;
+    bool ok = bb == 0.0;
+    while (!ok && outer < max_outer) {
+        rc = nd_convert_spinor(ctx64, r32, 32, r, 64);
+        if (rc != ND_OK) return rc;
+        ND_CUDA(ctx64, cudaStreamSynchronize(ctx64->stream));        // the fp32 context may run on another stream
+        int it = 0;
+        double ires = 0.0;
+        rc = nd_solve_DNm(ctx32, e32, r32, prefactor, mq, inner_tol, max_inner, iw, &ires, &it);   // synchronises
+        if (rc != ND_OK && rc != ND_ERR_NO_CONVERGENCE) return nd_fail(ctx64, rc, "solve_DNm_mixed: inner solve: %s", nd_last_error(ctx32));
+        inner_total += it;
+        rc = nd_convert_spinor(ctx64, e64, 64, e32, 32);
+        if (rc == ND_OK) rc = nd_axpy(ctx64, one, e64, x);
+        if (rc == ND_OK) rc = ndi_apply_DNm(ctx64, t, x, pa, pb, sw, 1);   // r = b - D x in fp64
+        if (rc == ND_OK) rc = nd_copy(ctx64, r, b);
+        if (rc == ND_OK) rc = nd_axpy(ctx64, m1, t, r);
+        if (rc == ND_OK) rc = nd_norm2(ctx64, r, &rr);
+        if (rc != ND_OK) return rc;
+        outer++;
+        ok = rr <= tol * tol * bb;
+    }
+    if (relres) *relres = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
+    if (stats) { stats[0] = outer; stats[1] = inner_total; }
+    if (!ok) return nd_fail(ctx64, ND_ERR_NO_CONVERGENCE, "solve_DNm_mixed: |b - D x|/|b| = %.3e > tol %.3e after %d outer steps", std::sqrt(rr / bb), tol, outer);
+    return ND_OK;
+}

@@ -72,3 +72,35 @@ def test_solve_fp32_and_failure_reporting():
     z = ctx.new_spinor()
     z.zero_()
     assert ctx.solve_DNm(x, z, RHO, mq) == (0.0, 0, True)
+
+
+def test_mixed_precision_refinement_reaches_fp64_accuracy():
+    """fp32 inner CG + fp64 residual (BASELINE config 4's 'fp32 inner, fp64 accumulation' applied to the inversion):
+    the solution must agree with the oracle's all-fp64 CG far below the fp32 floor, with a handful of fp64 applications."""
+    import paper_1010_5636_b200 as nd
+    from lattice_inputs import gauge_field
+
+    dims, n, eps, mq = (8, 4, 4, 8), 60, 0.004, 0.2
+    ctx64, DN = setup(64, dims, n, eps)
+    U = gauge_field(dims, "smooth", eps=0.3)
+    ctx32 = nd.Context(dims, prec=32, recon=12, bc_time=-1)
+    ctx32.set_gauge(U.astype(np.complex64))
+    ctx32.set_sign_poly(osign.cheb_coeffs(n, eps), eps, QNORM, M)
+    b = gaussian_spinor(dims)
+    x = ctx64.new_spinor()
+    relres, outer, inner, ok = ctx64.solve_DNm_mixed(ctx32, x, ctx64.pack_spinor(b), RHO, mq, tol=1e-10, inner_tol=1e-3)
+    assert ok and relres <= 1e-10 and 2 <= outer <= 8 and inner > outer
+    D = lambda v: osolver.apply_DNm(DN, v, 1.0 / RHO, mq)
+    Dd = lambda v: wilson.apply_gamma5(D(wilson.apply_gamma5(v)))
+    xr, _, _ = osolver.cg_normal_equations(D, Dd, b, 1e-12, 400)
+    got = ctx64.unpack_spinor(x)
+    assert rel_l2(got, xr) <= 1e-9
+    assert np.linalg.norm((b - D(got)).ravel()) <= 1e-9 * np.linalg.norm(b.ravel())
+    # precision conversion round trip and rejection of mismatched contexts
+    y32, y64 = ctx32.new_spinor(), ctx64.new_spinor()
+    ctx64.convert_spinor(y32, 32, x, 64)
+    ctx64.convert_spinor(y64, 64, y32, 32)
+    assert rel_l2(ctx64.unpack_spinor(y64), got) <= 1e-7
+    other = nd.Context((4, 4, 4, 4), prec=32, recon=12)
+    with pytest.raises(nd.NDError):
+        ctx64.solve_DNm_mixed(other, x, y64, RHO, mq)
