@@ -9,7 +9,8 @@
 //
 //   X = k = l + lextra Gaussian vectors, orthonormalised
 //   repeat:  X_j <- T_d((Q^2 - c)/e) X_j       [c-e, c+e] = [cut, qnorm^2] is damped, everything below cut amplified
-//            orthonormalise X  (Gram matrix, Hermitian eigendecomposition on the host, X <- X W Lambda^{-1/2}; twice)
+//            orthonormalise X  (Gram matrix, Hermitian eigendecomposition on the host, X <- X W Lambda^{-1/2}; repeated
+//                               when the Gram matrix is ill-conditioned)
 //            Rayleigh-Ritz of Q^2 in span X: H = X^dagger (Q^2 X), H = W Theta W^dagger, X <- X W
 //            residuals r_j = ||Q^2 x_j - theta_j x_j|| for j < l (computed explicitly), cut <- theta_{k-1}
 //   until max_j r_j <= tol
@@ -45,7 +46,7 @@ extern "C" int nd_heev(int k, const double* a_in, double* w, double* z_out) {
         double off = 0.0;
         for (int p = 0; p < k; p++)
             for (int q = p + 1; q < k; q++) off += std::norm(A[(size_t)p * k + q]);
-        if (std::sqrt(off) <= 1e-17 * scale * k) break;
+        if (std::sqrt(off) <= 1e-14 * scale * std::sqrt((double)k)) break;   // off-diagonal Frobenius norm at rounding level
         for (int p = 0; p < k; p++)
             for (int q = p + 1; q < k; q++) {
                 const zc apq = A[(size_t)p * k + q];
@@ -60,21 +61,26 @@ extern "C" int nd_heev(int k, const double* a_in, double* w, double* z_out) {
                 const double tau = (aqq - app) / (2.0 * b);
                 const double t = (tau >= 0.0 ? 1.0 : -1.0) / (std::fabs(tau) + std::sqrt(1.0 + tau * tau));
                 const double c = 1.0 / std::sqrt(1.0 + t * t), s = t * c;
-                const zc sp = s * ph, spc = s * std::conj(ph);   // s e^{i phi}, s e^{-i phi}
-                // A <- A J,  J = [[c, s e^{i phi}], [-s e^{-i phi}, c]] on columns (p, q)
+                const zc sp = s * ph;   // s e^{i phi}
+                // A <- A J,  J = [[c, s e^{i phi}], [-s e^{-i phi}, c]] on columns (p, q); Z <- Z J.  Written in real
+                // arithmetic: std::complex products go through the NaN-recovering library routine and run 10x slower.
+                const double sr = sp.real(), si = sp.imag();   // s e^{i phi} = sr + i si, s e^{-i phi} = sr - i si
+                auto rot_cols = [&](zc& ap, zc& aq) {
+                    const double pr = ap.real(), pi = ap.imag(), qr = aq.real(), qi = aq.imag();
+                    ap = zc(c * pr - (sr * qr + si * qi), c * pi - (sr * qi - si * qr));
+                    aq = zc((sr * pr - si * pi) + c * qr, (sr * pi + si * pr) + c * qi);
+                };
                 for (int i = 0; i < k; i++) {
-                    const zc xp = A[(size_t)i * k + p], xq = A[(size_t)i * k + q];
-                    A[(size_t)i * k + p] = c * xp - spc * xq;
-                    A[(size_t)i * k + q] = sp * xp + c * xq;
-                    const zc zp = Z[(size_t)i * k + p], zq = Z[(size_t)i * k + q];
-                    Z[(size_t)i * k + p] = c * zp - spc * zq;
-                    Z[(size_t)i * k + q] = sp * zp + c * zq;
+                    rot_cols(A[(size_t)i * k + p], A[(size_t)i * k + q]);
+                    rot_cols(Z[(size_t)i * k + p], Z[(size_t)i * k + q]);
                 }
-                // A <- J^dagger A on rows (p, q)
+                // A <- J^dagger A on rows (p, q): row_p <- c row_p - s e^{i phi} row_q, row_q <- s e^{-i phi} row_p + c row_q
+                zc* rp = &A[(size_t)p * k];
+                zc* rq = &A[(size_t)q * k];
                 for (int j = 0; j < k; j++) {
-                    const zc xp = A[(size_t)p * k + j], xq = A[(size_t)q * k + j];
-                    A[(size_t)p * k + j] = c * xp - sp * xq;
-                    A[(size_t)q * k + j] = spc * xp + c * xq;
+                    const double pr = rp[j].real(), pi = rp[j].imag(), qr = rq[j].real(), qi = rq[j].imag();
+                    rp[j] = zc(c * pr - (sr * qr - si * qi), c * pi - (sr * qi + si * qr));
+                    rq[j] = zc((sr * pr + si * pi) + c * qr, (sr * pi - si * pr) + c * qi);
                 }
                 A[(size_t)p * k + q] = A[(size_t)q * k + p] = 0.0;
                 A[(size_t)p * k + p] = A[(size_t)p * k + p].real();
@@ -190,6 +196,8 @@ struct Solver {
             rc = rotate(Y, k, X, k, C);
             if (rc != ND_OK) return rc;
             std::swap(X, Y);
+            // the loss of orthogonality of X W Lambda^{-1/2} is ~ rounding * cond(Gram): a second pass only when needed
+            if (w[k - 1] / w[0] < (ctx->prec == 32 ? 30.0 : 1.0e6)) break;
         }
         return ND_OK;
     }
