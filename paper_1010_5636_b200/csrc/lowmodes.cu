@@ -12,7 +12,8 @@
 //            orthonormalise X  (Gram matrix, Hermitian eigendecomposition on the host, X <- X W Lambda^{-1/2}; repeated
 //                               when the Gram matrix is ill-conditioned)
 //            Rayleigh-Ritz of Q^2 in span X: H = X^dagger (Q^2 X), H = W Theta W^dagger, X <- X W
-//            residuals r_j = ||Q^2 x_j - theta_j x_j|| for j < l (computed explicitly), cut <- theta_{k-1}
+//            residuals r_j = ||Q^2 x_j - theta_j x_j|| for j < l (computed explicitly), cut <- theta_{k-1};
+//            leading columns with r_j <= tol/2 are locked (not filtered again)
 //   until max_j r_j <= tol
 //   Rayleigh-Ritz of Q in the span of the l lowest x_j: M = X^dagger Q X -> (nu_k, u_k), rho_k = ||(Q - nu_k) u_k||   (2.7, 2.8)
 //
@@ -202,9 +203,11 @@ struct Solver {
         return ND_OK;
     }
     // X_j <- T_d((Q^2 - c)/e) X_j, d even; t_{i+1} = (2/e)(Q^2 - c) t_i - t_{i-1}, the update folded into the 2nd stencil
-    int filter(int d, double lo, double hi) {
+    // columns j < first are locked (their residual met the tolerance): they stay in the block for the orthonormalisation
+    // and the Rayleigh-Ritz step but are not filtered again
+    int filter(int d, double lo, double hi, int first) {
         const double c = 0.5 * (hi + lo), e = 0.5 * (hi - lo);
-        for (int j = 0; j < k; j++) {
+        for (int j = first; j < k; j++) {
             char* P = x(j);   // t_{i-1}
             char* R = s0;     // t_i
             int rc = Q(s1, P);
@@ -275,9 +278,10 @@ extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, d
     rc = S.orthonormalise(2);
     if (rc != ND_OK) return finish(rc);
     double cut = -1.0;   // unknown before the first Rayleigh-Ritz step
+    int nlock = 0;
     for (it = 0; it <= maxit; it++) {
         if (it > 0) {
-            rc = S.filter(d, cut, hi);
+            rc = S.filter(d, cut, hi, nlock);
             if (rc != ND_OK) return finish(rc);
             rc = S.orthonormalise(2);
             if (rc != ND_OK) return finish(rc);
@@ -306,6 +310,8 @@ extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, d
             worst = std::max(worst, rq[j]);
         }
         if (worst <= tol) { converged = true; break; }
+        nlock = 0;
+        while (nlock < l && rq[nlock] <= 0.5 * tol) nlock++;   // leading Ritz pairs already well inside the tolerance
         // damp everything above the block's largest Ritz value next time (keep the interval non-degenerate)
         cut = std::min(theta[k - 1], 0.5 * hi);
         if (lextra == 0) cut = std::min(theta[k - 1] * 1.05 + 1e-3, 0.5 * hi);
