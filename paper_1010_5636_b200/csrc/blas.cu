@@ -179,6 +179,96 @@ __global__ void __launch_bounds__(RED_THREADS) block_axpy_kernel(typename Prec<T
     }
 }
 
+// ----------------------------------------------------------------------------------- grouped Gram / rotation
+// The eigen-solver needs X^dagger Y and X C for blocks of k vectors (lowmodes.cu).  Column by column (block_dot /
+// block_axpy) the block X is re-read k times.  These two kernels take NG columns at a time, so X is streamed k/NG times.
+//
+// gram: partial[((j*l + k)*2 + c)][block] = sum over the block's sites of conj(v_k) x_j, j < ng <= NG.  The loop over
+// k is OUTSIDE the loop over the CTA's sites: the NG x-columns of those sites are re-read from L1/L2, v_k is streamed
+// once, and the accumulators of one k fit in registers, so there is one warp reduction per k and not one per chunk.
+template <typename T, int NG>
+__global__ void __launch_bounds__(RED_THREADS) block_gram_kernel(double* __restrict__ partial, int l, int ng,
+                                                                 const typename Prec<T>::Vec* __restrict__ v,
+                                                                 const typename Prec<T>::Vec* __restrict__ x, long long V) {
+    __shared__ double sm[RED_WARPS][2 * NG];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long nchunks = (V + blockDim.x - 1) / blockDim.x;
+    for (int k = 0; k < l; k++) {
+        double re[NG], im[NG];
+#pragma unroll
+        for (int j = 0; j < NG; j++) re[j] = im[j] = 0.0;
+        const typename Prec<T>::Vec* vk = v + (long long)k * Prec<T>::NV * V;
+        for (long long ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
+            const long long s = ch * blockDim.x + threadIdx.x;
+            if (s >= V) continue;
+            cx<T> b[12];
+            load_site<T>(vk, V, s, b);
+#pragma unroll
+            for (int j = 0; j < NG; j++) {
+                if (j < ng) {
+                    cx<T> a[12];
+                    load_site<T>(x + (long long)j * Prec<T>::NV * V, V, s, a);
+#pragma unroll
+                    for (int i = 0; i < 12; i++) {
+                        const double br = (double)b[i].re, bi = (double)b[i].im, xr = (double)a[i].re, xi = (double)a[i].im;
+                        re[j] = fma(br, xr, re[j]);
+                        re[j] = fma(bi, xi, re[j]);
+                        im[j] = fma(br, xi, im[j]);
+                        im[j] = fma(-bi, xr, im[j]);
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < NG; j++) {
+            re[j] = warp_sum(re[j]);
+            im[j] = warp_sum(im[j]);
+            if (lane == 0) { sm[warp][2 * j] = re[j]; sm[warp][2 * j + 1] = im[j]; }
+        }
+        __syncthreads();
+        if (threadIdx.x < 2 * ng) {
+            double t = 0.0;
+#pragma unroll
+            for (int w = 0; w < RED_WARPS; w++) t += sm[w][threadIdx.x];
+            const int j = threadIdx.x >> 1, c = threadIdx.x & 1;
+            partial[((long long)(j * l + k) * 2 + c) * gridDim.x + blockIdx.x] = t;
+        }
+        __syncthreads();
+    }
+}
+
+// rotate: y_j = sum_{i < l} coef[j*l + i] v_i for j < ng <= NG output columns (y_j at y + j*NV*V), one pass over v
+template <typename T, int NG>
+__global__ void __launch_bounds__(RED_THREADS) block_rotate_kernel(typename Prec<T>::Vec* __restrict__ y, int l, int ng,
+                                                                   const double* __restrict__ coef,
+                                                                   const typename Prec<T>::Vec* __restrict__ v, long long V) {
+    extern __shared__ double sm[];   // [NG][2l]
+    for (int i = threadIdx.x; i < 2 * l * ng; i += blockDim.x) sm[i] = coef[i];
+    __syncthreads();
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < V; s += (long long)gridDim.x * blockDim.x) {
+        cx<T> acc[NG][12];
+#pragma unroll
+        for (int j = 0; j < NG; j++)
+#pragma unroll
+            for (int i = 0; i < 12; i++) acc[j][i] = {T(0), T(0)};
+        for (int k = 0; k < l; k++) {
+            cx<T> b[12];
+            load_site<T>(v + (long long)k * Prec<T>::NV * V, V, s, b);
+#pragma unroll
+            for (int j = 0; j < NG; j++) {
+                if (j < ng) {
+                    const cx<T> a = {(T)sm[(j * l + k) * 2], (T)sm[(j * l + k) * 2 + 1]};
+#pragma unroll
+                    for (int i = 0; i < 12; i++) cfma(acc[j][i], a, b[i]);
+                }
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < NG; j++)
+            if (j < ng) store_site<T>(y + (long long)j * Prec<T>::NV * V, V, s, acc[j]);
+    }
+}
+
 // --------------------------------------------------------------------------------------------- gaussian
 __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0, unsigned k1,
                                               unsigned (&out)[4]) {
@@ -277,6 +367,41 @@ int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, 
         else block_axpy_kernel<double, 1><<<blocks, RED_THREADS, smem, ctx->stream>>>((Vec*)y, l, d_coef, (const Vec*)v, (const Vec*)eta, pa, pb, ctx->V);
     }
     ND_LAUNCHED(ctx);
+    return ND_OK;
+}
+
+// G[k][j] = <v_k, x_j>, k < l, j < nx, into d_out[(j*l + k)*2 + {re, im}] (device); x_j at x + j*spinor_bytes
+int ndi_block_gram_dev(nd_ctx* ctx, int l, const void* v, int nx, const void* x, double* d_out) {
+    const size_t sb = nd_spinor_bytes(ctx);
+    const int NG = ctx->prec == 32 ? 8 : 4;
+    // the partial-sum scratch holds ND_RESULT_DOUBLES x ND_MAX_RED_BLOCKS doubles: rows (2 l NG) x blocks must fit
+    long long cap = (long long)ND_RESULT_DOUBLES * ND_MAX_RED_BLOCKS / ((long long)2 * l * NG);
+    if (cap > 4 * ctx->num_sms) cap = 4 * ctx->num_sms;
+    const unsigned blocks = grid_for(ctx->V, RED_THREADS, (int)cap);
+    for (int j0 = 0; j0 < nx; j0 += NG) {
+        const int ng = nx - j0 < NG ? nx - j0 : NG;
+        const char* xj = (const char*)x + (size_t)j0 * sb;
+        if (ctx->prec == 32) block_gram_kernel<float, 8><<<blocks, RED_THREADS, 0, ctx->stream>>>(ctx->d_partial, l, ng, (const float4*)v, (const float4*)xj, ctx->V);
+        else block_gram_kernel<double, 4><<<blocks, RED_THREADS, 0, ctx->stream>>>(ctx->d_partial, l, ng, (const double2*)v, (const double2*)xj, ctx->V);
+        ND_LAUNCHED(ctx);
+        reduce_partials_kernel<<<ng * l * 2, RED_THREADS, 0, ctx->stream>>>(d_out + (size_t)2 * l * j0, ctx->d_partial, (int)blocks);
+        ND_LAUNCHED(ctx);
+    }
+    return ND_OK;
+}
+// y_j = sum_i coef[j*l + i] v_i for j < ny (coef: ny*l complex doubles on the device, y_j at y + j*spinor_bytes)
+int ndi_block_rotate_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, int ny, void* y) {
+    const size_t sb = nd_spinor_bytes(ctx);
+    const int NG = ctx->prec == 32 ? 4 : 2;
+    const unsigned blocks = grid_for(ctx->V, RED_THREADS, 1 << 30);
+    for (int j0 = 0; j0 < ny; j0 += NG) {
+        const int ng = ny - j0 < NG ? ny - j0 : NG;
+        char* yj = (char*)y + (size_t)j0 * sb;
+        const size_t smem = (size_t)2 * l * ng * sizeof(double);
+        if (ctx->prec == 32) block_rotate_kernel<float, 4><<<blocks, RED_THREADS, smem, ctx->stream>>>((float4*)yj, l, ng, d_coef + (size_t)2 * l * j0, (const float4*)v, ctx->V);
+        else block_rotate_kernel<double, 2><<<blocks, RED_THREADS, smem, ctx->stream>>>((double2*)yj, l, ng, d_coef + (size_t)2 * l * j0, (const double2*)v, ctx->V);
+        ND_LAUNCHED(ctx);
+    }
     return ND_OK;
 }
 

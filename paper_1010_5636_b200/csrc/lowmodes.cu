@@ -5,7 +5,7 @@
 // are given.  DESIGN.md reading R13: any method delivering ||Q^2 x - theta x|| <= tol with orthonormal x.  Built here:
 // Chebyshev-filtered block subspace iteration, which minimises the block Ritz functional tr(X^dagger Q^2 X) over
 // orthonormal blocks X and is made of exactly the kernels D_N uses (plain stencil, stencil with the fused three-term
-// epilogue, block dot, block axpy):
+// epilogue, block dot, grouped Gram / rotation kernels):
 //
 //   X = k = l + lextra Gaussian vectors, orthonormalised
 //   repeat:  X_j <- T_d((Q^2 - c)/e) X_j       [c-e, c+e] = [cut, qnorm^2] is damped, everything below cut amplified
@@ -148,10 +148,8 @@ struct Solver {
     }
     // G[i][j] = <A_i, B_j>, i < na, j < nb  -> h_mat row-major (na x nb complex)
     int gram(char* A, int na, char* B, int nb) {
-        for (int j = 0; j < nb; j++) {
-            int rc = ndi_block_dot_dev(ctx, na, A, B + (size_t)j * sb, d_mat + (size_t)2 * na * j);
-            if (rc != ND_OK) return rc;
-        }
+        int rc = ndi_block_gram_dev(ctx, na, A, nb, B, d_mat);   // d_mat[(j*na + i)*2 + c] = <A_i, B_j>
+        if (rc != ND_OK) return rc;
         std::vector<double> tmp((size_t)2 * na * nb);
         ND_CUDA(ctx, cudaMemcpyAsync(tmp.data(), d_mat, tmp.size() * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
         ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -173,12 +171,7 @@ struct Solver {
             }
         ND_CUDA(ctx, cudaMemcpyAsync(d_mat, col.data(), col.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
         ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));   // `col` is pageable and dies with this frame
-        ND_CUDA(ctx, cudaMemsetAsync(dst, 0, (size_t)nd * sb, ctx->stream));
-        for (int j = 0; j < nd; j++) {
-            int rc = ndi_block_axpy_dev(ctx, ns, d_mat + (size_t)2 * ns * j, src, dst + (size_t)j * sb, 0, nullptr, 0.0, 0.0);
-            if (rc != ND_OK) return rc;
-        }
-        return ND_OK;
+        return ndi_block_rotate_dev(ctx, ns, d_mat, src, nd, dst);
     }
     // X <- X W Lambda^{-1/2} with X^dagger X = W Lambda W^dagger (result back in X)
     int orthonormalise(int reps) {

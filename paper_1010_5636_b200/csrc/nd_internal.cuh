@@ -154,6 +154,8 @@ int ndi_block_dot2_dev(nd_ctx* ctx, int l, const void* v, const void* x0, const 
 int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pa,
                        double pb);   // mode 1: y <- pa*eta + pb*gamma5(y + sum_k a_k v_k)
 int ndi_apply_DNm(nd_ctx* ctx, void* out, const void* in, double pa, double pb, void* work, int use_graph);
+int ndi_block_gram_dev(nd_ctx* ctx, int l, const void* v, int nx, const void* x, double* d_out);      // d_out[(j*l+k)*2+c]
+int ndi_block_rotate_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, int ny, void* y);  // coef[(j*l+i)*2+c]
 int ndi_read_result(nd_ctx* ctx, const double* d_src, double* h_dst, int n);              // sync copy to host
 int ndi_drop_graphs(nd_ctx* ctx);
 constexpr int ND_RESULT_DOUBLES = 4 * ND_MAX_BLOCK_L;
