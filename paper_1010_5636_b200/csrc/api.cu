@@ -74,6 +74,7 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
         for (int i = 0; i < 3; i++) ctx->tile_lb[i] = lb[i];
         ctx->tile_threads = (threads >= 64 && !(e && e[0] == '0' && e[1] == 0)) ? threads : 0;
     }
+    ctx->hop_max_sites = getenv("ND_HOP_MAX") ? atoi(getenv("ND_HOP_MAX")) : 16384;
     ctx->num_sms = 148;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     ctx->err[0] = 0;

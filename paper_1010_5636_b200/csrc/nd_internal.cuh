@@ -56,6 +56,7 @@ struct nd_ctx {
     long long launches;
     bool capturing;
     int num_sms;
+    int hop_max_sites;  // lattices below this volume use the hop-parallel stencil (wilson.cu)
     int tile_lb[3];     // stencil CTA tile: log2 extents along x1, x2, x3
     int tile_threads;   // sites per tile (0: linear mapping)
     char err[512];

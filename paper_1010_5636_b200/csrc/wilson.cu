@@ -236,6 +236,102 @@ __global__ void __launch_bounds__(ND_Q_THREADS, q_min_blocks<T>()) wilson_Q_kern
     finish_site<T, EPI>(out, G.V, s, acc, s0, s1, v1, s2, v2, s3, v3);
 }
 
+// --------------------------------------------------------------------------------- hop-parallel kernel (tiny lattices)
+// On lattices of a few thousand sites (BASELINE config 3, 8^3x16) there are fewer sites than the GPU has lanes and the
+// stencil is bound by the latency of its chain of eight dependent load -> multiply steps.  Here a CTA is 8 warps x 32
+// sites: warp h computes hop h (h = 2 mu + {0: forward, 1: backward}) of the same 32 sites, so every load of a site is
+// in flight at once; the eight contributions are summed through shared memory and warp p finishes plane p (mass term,
+// gamma5, fused epilogue, one coalesced 128-bit store).
+template <typename T, int RECON, int MU, int SGN>
+__device__ __forceinline__ void single_hop(const typename Prec<T>::Vec* __restrict__ in,
+                                           const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, long long V,
+                                           long long s_spinor, long long s_link, T phase, cx<T> (&acc)[12]) {
+    cx<T> psi[12], U[3][3], h[2][3], g[2][3];
+    load_spinor<T>(in, V, s_spinor, psi);
+    load_link<T, RECON>(gauge, V, MU, s_link, U);
+    project<T, MU, SGN>(psi, phase, h);
+    if (SGN < 0) mul_U(U, h, g);
+    else mul_Udag(U, h, g);
+    accumulate<T, MU, SGN>(g, acc);
+}
+
+template <typename T, int RECON, bool EPI>
+__global__ void __launch_bounds__(256) wilson_Q_hop_kernel(typename Prec<T>::Vec* __restrict__ out,
+                                                           const typename Prec<T>::Vec* __restrict__ in,
+                                                           const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, Geom G,
+                                                           T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2,
+                                                           const typename Prec<T>::Vec* v2, T s3,
+                                                           const typename Prec<T>::Vec* v3) {
+    using Vec = typename Prec<T>::Vec;
+    constexpr int NV = Prec<T>::NV;
+    constexpr int W = 24 / NV;   // reals per 128-bit word
+    __shared__ T red[8][24][32];
+    const int lane = threadIdx.x, hop = threadIdx.y;
+    const long long s = (long long)blockIdx.x * 32 + lane;
+    const bool valid = s < G.V;
+    cx<T> acc[12];
+#pragma unroll
+    for (int i = 0; i < 12; i++) acc[i] = {T(0), T(0)};
+    if (valid) {
+        const int x3 = (int)(s % G.L3);
+        long long r = s / G.L3;
+        const int x2 = (int)(r % G.L2);
+        r /= G.L2;
+        const int x1 = (int)(r % G.L1);
+        const int x0 = (int)(r / G.L1);
+        switch (hop) {   // warp-uniform
+            case 0: single_hop<T, RECON, 0, -1>(in, gauge, G.V, (x0 == G.L0 - 1) ? s - (long long)(G.L0 - 1) * G.S0 : s + G.S0, s,
+                                                 (x0 == G.L0 - 1) ? T(G.bc) : T(1), acc); break;
+            case 1: { const long long sb = (x0 == 0) ? s + (long long)(G.L0 - 1) * G.S0 : s - G.S0;
+                      single_hop<T, RECON, 0, +1>(in, gauge, G.V, sb, sb, (x0 == 0) ? T(G.bc) : T(1), acc); } break;
+            case 2: single_hop<T, RECON, 1, -1>(in, gauge, G.V, (x1 == G.L1 - 1) ? s - (long long)(G.L1 - 1) * G.S1 : s + G.S1, s, T(1), acc); break;
+            case 3: { const long long sb = (x1 == 0) ? s + (long long)(G.L1 - 1) * G.S1 : s - G.S1;
+                      single_hop<T, RECON, 1, +1>(in, gauge, G.V, sb, sb, T(1), acc); } break;
+            case 4: single_hop<T, RECON, 2, -1>(in, gauge, G.V, (x2 == G.L2 - 1) ? s - (long long)(G.L2 - 1) * G.S2 : s + G.S2, s, T(1), acc); break;
+            case 5: { const long long sb = (x2 == 0) ? s + (long long)(G.L2 - 1) * G.S2 : s - G.S2;
+                      single_hop<T, RECON, 2, +1>(in, gauge, G.V, sb, sb, T(1), acc); } break;
+            case 6: single_hop<T, RECON, 3, -1>(in, gauge, G.V, (x3 == G.L3 - 1) ? s - (G.L3 - 1) : s + 1, s, T(1), acc); break;
+            default: { const long long sb = (x3 == 0) ? s + (G.L3 - 1) : s - 1;
+                       single_hop<T, RECON, 3, +1>(in, gauge, G.V, sb, sb, T(1), acc); } break;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 12; i++) {
+        red[hop][2 * i][lane] = acc[i].re;
+        red[hop][2 * i + 1][lane] = acc[i].im;
+    }
+    __syncthreads();
+    if (!valid) return;
+    for (int p = hop; p < NV; p += 8) {   // warp `hop` finishes planes hop, hop + 8
+        Vec phi = in[p * G.V + s], w;
+        const T* pr = reinterpret_cast<const T*>(&phi);
+        T* wr = reinterpret_cast<T*>(&w);
+        const T sg = (p * W < 12) ? T(1) : T(-1);   // gamma5: reals 0..11 are spin 0, 1
+#pragma unroll
+        for (int k = 0; k < W; k++) {
+            T t = T(0);
+#pragma unroll
+            for (int h = 0; h < 8; h++) t += red[h][p * W + k][lane];
+            wr[k] = sg * fma(T(-0.5), t, mass_term * pr[k]);
+        }
+        if (EPI) {
+#pragma unroll
+            for (int k = 0; k < W; k++) wr[k] *= s0;
+            const Vec* vs[3] = {v1, v2, v3};
+            const T ss[3] = {s1, s2, s3};
+#pragma unroll
+            for (int j = 0; j < 3; j++)
+                if (vs[j]) {
+                    Vec a = vs[j][p * G.V + s];
+                    const T* ar = reinterpret_cast<const T*>(&a);
+#pragma unroll
+                    for (int k = 0; k < W; k++) wr[k] = fma(ss[j], ar[k], wr[k]);
+                }
+        }
+        out[p * G.V + s] = w;
+    }
+}
+
 template <typename T, int RECON>
 int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
              const void* v2, double s3, const void* v3) {
@@ -248,7 +344,22 @@ int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double 
     G.S1 = (long long)G.L2 * G.L3;
     G.S0 = (long long)G.L1 * G.L2 * G.L3;
     G.bc = ctx->bc;
-    // 128 threads per CTA; small lattices (launch-latency-bound, BASELINE config 3) get smaller CTAs so that every SM has work
+    if (ctx->V < (long long)ctx->hop_max_sites) {
+        // fewer sites than lanes on the chip: one warp per hop (latency-bound regime, BASELINE config 3)
+        const unsigned nb = (unsigned)((ctx->V + 31) / 32);
+        const dim3 tb(32, 8, 1);
+        if (epi)
+            wilson_Q_hop_kernel<T, RECON, true><<<nb, tb, 0, ctx->stream>>>(
+                (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(s0), T(s1), (const Vec*)v1, T(s2),
+                (const Vec*)v2, T(s3), (const Vec*)v3);
+        else
+            wilson_Q_hop_kernel<T, RECON, false><<<nb, tb, 0, ctx->stream>>>(
+                (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(1), T(0), nullptr, T(0), nullptr, T(0),
+                nullptr);
+        ND_LAUNCHED(ctx);
+        return ND_OK;
+    }
+    // 128 threads per CTA; small lattices get smaller CTAs so that every SM has work
     int threads = 128;
     while (threads > 32 && ctx->V / threads < 2 * ctx->num_sms) threads /= 2;
     unsigned blocks = (unsigned)((ctx->V + threads - 1) / threads);
