@@ -82,8 +82,11 @@ ND_API long long nd_launch_count(const nd_ctx* ctx);
 ND_API int nd_set_gauge(nd_ctx* ctx, const void* links_aos, int src_prec, int on_device);
 ND_API int nd_get_gauge(nd_ctx* ctx, void* links_aos_c128, int on_device);
 /* Diagnostics of the last nd_set_gauge: out[0] = max |U^dagger U - 1| entry, out[1] = max |det U - 1|,
- * out[2] = min over links of N = |a2|^2 + |a3|^2 (conditioning of the 8-parameter form). */
-ND_API int nd_gauge_stats(nd_ctx* ctx, double out[3]);
+ * out[2] = min over links of N = |a2|^2 + |a3|^2 (conditioning of the 8-parameter form), out[3] = max entry of
+ * |reconstruct(stored parameters) - U| (what the stencil will see; with recon 8 rounding is amplified by ~1/N and
+ * nd_set_gauge returns ND_ERR_RECON8_SINGULAR above 2e-3 (fp32) / 1e-8 (fp64)).  A NaN anywhere in the links makes
+ * out[0] = out[1] = +inf and nd_set_gauge fail with ND_ERR_NOT_SU3. */
+ND_API int nd_gauge_stats(nd_ctx* ctx, double out[4]);
 
 /* ------------------------------------------------------------------------------------------------ layout
  * Canonical AoS (prec 32: complex64 / 64: complex128; host or device) <-> device SoA in the context's

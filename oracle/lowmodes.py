@@ -104,3 +104,35 @@ def projector_bound(kappa):
     +inf when the denominator is not positive (the bound says nothing there)."""
     x = 2.0 * kappa * (1.0 + 2.0 * kappa)
     return float(kappa * (1.0 + 2.0 * kappa) / (1.0 - x)) if x < 1.0 else float("inf")
+
+
+# ----------------------------------------------------------------------------- dynamic choice of l, PAPER.md:L110
+def choose_l(abs_nu, l_min, l_max):
+    """"The number of low modes included in the projector will be determined dynamically in such a way that the
+    spectral distance from the other modes is not accidentally small".  Reading (R17): given
+    the moduli |nu_1| <= |nu_2| <= ... of the Ritz values of Q in the block (projected candidates AND guard vectors),
+    the cut l' in [l_min, l_max] is put at the LARGEST gap |nu_{l'+1}| - |nu_{l'}|; ties go to the smallest l'.
+    Needs len(abs_nu) >= l_max + 1 (at least one value beyond the last candidate)."""
+    a = np.asarray(abs_nu, dtype=np.float64)
+    assert np.all(np.diff(a) >= 0) and 1 <= l_min <= l_max < len(a)
+    best, best_gap = l_min, -1.0
+    for l in range(l_min, l_max + 1):
+        gap = a[l] - a[l - 1]
+        if gap > best_gap:
+            best, best_gap = l, gap
+    return best, best_gap
+
+
+def error_control(nu_block, rho_block, l_min, l_max):
+    """The whole error control of PAPER.md:L86-110 on a block of Ritz pairs of Q sorted by |nu| (eq. 2.8 residues
+    rho given): choose l' by `choose_l`; d_k (L90) from the Ritz values outside the cut - the guard values |nu_j|,
+    j >= l', taken with BOTH signs because a poorly converged guard vector does not fix its sign - and from the
+    projected values of the opposite sign; kappa_+- (2.9); bound (2.10).  Returns dict(l, gap, d, kappa, bound)."""
+    nu = np.asarray(nu_block, dtype=np.float64)
+    rho = np.asarray(rho_block, dtype=np.float64)
+    a = np.abs(nu)
+    l, gap = choose_l(a, l_min, l_max)
+    rest = np.concatenate([a[l:], -a[l:]])
+    d = distances_d(nu[:l], rest)
+    kp, km = kappa_pm(nu[:l], rho[:l], d)
+    return dict(l=l, gap=gap, d=d, kappa=(kp, km), bound=(projector_bound(kp), projector_bound(km)))

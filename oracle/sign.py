@@ -126,8 +126,3 @@ def apply_DN(Q, gamma5, eta, c, eps, qnorm, prefactor, nu=None, U=None):
         s = sign_projected(Q, eta, c, eps, qnorm, nu, U)
     return prefactor * (eta + gamma5(s))
 
-
-def exact_sign_dense(Qmat):
-    """sign(Q) = W sign(Lambda) W^dagger from the dense Hermitian eigendecomposition (4^4 pin, P8)."""
-    lam, W = np.linalg.eigh(Qmat)
-    return (W * np.sign(lam)) @ W.conj().T, lam, W

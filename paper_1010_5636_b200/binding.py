@@ -236,7 +236,7 @@ class Context:
         return out
 
     def gauge_stats(self):
-        out = (ctypes.c_double * 3)()
+        out = (ctypes.c_double * 4)()
         self._chk(self.lib.nd_gauge_stats(self._h, out))
         return tuple(out)
 

@@ -16,10 +16,9 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnd_b200.so")
 SOURCES = ["api.cu", "layout.cu", "wilson.cu", "blas.cu", "sign.cu", "lowmodes.cu", "solver.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+# IEEE arithmetic: no --use_fast_math anywhere
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false"]
-FLAGS = [f for f in FLAGS if f != "--use_fast_math=false"]   # IEEE arithmetic: never fast-math
-FLAGS += os.environ.get("ND_NVCC_EXTRA", "").split()        # tuning sweeps only (e.g. -DND_MINB32=6)
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
 
 def _deps():

@@ -43,7 +43,7 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->stream = (cudaStream_t)stream;
     ctx->gauge = nullptr;
     ctx->gauge_set = false;
-    ctx->gstats[0] = ctx->gstats[1] = ctx->gstats[2] = 0.0;
+    ctx->gstats[0] = ctx->gstats[1] = ctx->gstats[2] = ctx->gstats[3] = 0.0;
     ctx->d_partial = ctx->d_result = ctx->h_result = ctx->d_coef = ctx->d_nu = nullptr;
     ctx->n = 0;
     ctx->eps = ctx->qnorm = ctx->m_sign = 0.0;
@@ -54,14 +54,11 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->capturing = false;
     {
         // stencil CTA tile (x1, x2, x3) of 128 sites: x3 extent = the largest power of two <= 32 dividing L3, then x2 and
-        // x1 are doubled in turn while they divide the lattice (32^3: 2 x 2 x 32).  ND_TILE="b1,b2,b3" caps the extents
-        // (tuning only), "0" forces the linear mapping; lattices without a tile of >= 64 sites use the linear mapping.
-        int cap[3] = {128, 128, 32};
-        const char* e = getenv("ND_TILE");
-        if (e) sscanf(e, "%d,%d,%d", &cap[0], &cap[1], &cap[2]);
+        // x1 are doubled in turn while they divide the lattice (32^3: 2 x 2 x 32); lattices without a tile of >= 64 sites
+        // use the linear mapping.
         int lb[3] = {0, 0, 0}, threads = 1;
         auto grow = [&](int i) {
-            if (threads * 2 > 128 || (2 << lb[i]) > cap[i] || dims[i + 1] % (2 << lb[i]) != 0) return false;
+            if (threads * 2 > 128 || (2 << lb[i]) > (i == 2 ? 32 : 128) || dims[i + 1] % (2 << lb[i]) != 0) return false;
             lb[i]++;
             threads *= 2;
             return true;
@@ -72,9 +69,9 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
             g = grow(0) || g;
         }
         for (int i = 0; i < 3; i++) ctx->tile_lb[i] = lb[i];
-        ctx->tile_threads = (threads >= 64 && !(e && e[0] == '0' && e[1] == 0)) ? threads : 0;
+        ctx->tile_threads = (threads >= 64) ? threads : 0;
     }
-    ctx->hop_max_sites = getenv("ND_HOP_MAX") ? atoi(getenv("ND_HOP_MAX")) : 16384;
+    ctx->hop_max_sites = 16384;   // below this volume there are fewer sites than lanes: hop-parallel stencil (wilson.cu)
     ctx->num_sms = 148;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     ctx->err[0] = 0;

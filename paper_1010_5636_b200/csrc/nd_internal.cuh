@@ -36,7 +36,7 @@ struct nd_ctx {
     void* gauge;
     size_t gauge_bytes;
     bool gauge_set;
-    double gstats[3];
+    double gstats[4];
     // reductions
     double* d_partial;   // [ND_MAX_RED_BLOCKS * 2 * ND_MAX_BLOCK_L]
     double* d_result;    // [2 * ND_MAX_BLOCK_L * 2]

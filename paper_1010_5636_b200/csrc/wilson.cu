@@ -115,9 +115,10 @@ __device__ __forceinline__ void hop_pair(const typename Prec<T>::Vec* __restrict
 }
 
 // out(x) = gamma5 [ -1/2 acc ] (acc holds -2 (4+m) phi(x) + the eight hops), optionally followed by the fused vector update
-// out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3 (every v_i(x) is read before the store, so out may alias them)
+// out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3.  out may alias any v_i (the Clenshaw step passes v2 == out): neither out nor the
+// v_i are __restrict__, every v_i(x) is read before out(x) is written, and no other thread touches site x.
 template <typename T, bool EPI>
-__device__ __forceinline__ void finish_site(typename Prec<T>::Vec* __restrict__ out, long long V, long long s,
+__device__ __forceinline__ void finish_site(typename Prec<T>::Vec* out, long long V, long long s,
                                             const cx<T> (&acc)[12], T s0, T s1,
                                             const typename Prec<T>::Vec* v1, T s2, const typename Prec<T>::Vec* v2, T s3,
                                             const typename Prec<T>::Vec* v3) {
@@ -156,20 +157,12 @@ __device__ __forceinline__ void finish_site(typename Prec<T>::Vec* __restrict__ 
     for (int p = 0; p < NV; p++) out[p * V + s] = w[p];
 }
 
-#ifndef ND_Q_THREADS
-#define ND_Q_THREADS 128
-#endif
-#ifndef ND_MINB32
-#define ND_MINB32 5
-#endif
-#ifndef ND_MINB64
-#define ND_MINB64 3
-#endif
-// resident CTAs per SM the register allocation is tuned for (fp32 / fp64)
-template <typename T> constexpr int q_min_blocks() { return sizeof(T) == 4 ? ND_MINB32 : ND_MINB64; }
+// 128 threads per CTA; resident CTAs per SM the register allocation is tuned for: 5 (fp32, 96 registers) / 3 (fp64, 168)
+constexpr int Q_THREADS = 128;
+template <typename T> constexpr int q_min_blocks() { return sizeof(T) == 4 ? 5 : 3; }
 
 template <typename T, int RECON, bool EPI>
-__global__ void __launch_bounds__(ND_Q_THREADS, q_min_blocks<T>()) wilson_Q_kernel(typename Prec<T>::Vec* __restrict__ out,
+__global__ void __launch_bounds__(Q_THREADS, q_min_blocks<T>()) wilson_Q_kernel(typename Prec<T>::Vec* out,
                                                        const typename Prec<T>::Vec* __restrict__ in,
                                                        const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, Geom G,
                                                        T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2,
@@ -256,7 +249,7 @@ __device__ __forceinline__ void single_hop(const typename Prec<T>::Vec* __restri
 }
 
 template <typename T, int RECON, bool EPI>
-__global__ void __launch_bounds__(256) wilson_Q_hop_kernel(typename Prec<T>::Vec* __restrict__ out,
+__global__ void __launch_bounds__(256) wilson_Q_hop_kernel(typename Prec<T>::Vec* out,
                                                            const typename Prec<T>::Vec* __restrict__ in,
                                                            const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, Geom G,
                                                            T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2,
@@ -364,7 +357,7 @@ int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double 
     while (threads > 32 && ctx->V / threads < 2 * ctx->num_sms) threads /= 2;
     unsigned blocks = (unsigned)((ctx->V + threads - 1) / threads);
     for (int i = 0; i < 3; i++) { G.lb[i] = ctx->tile_lb[i]; G.nt[i] = 0; }
-    if (ctx->tile_threads > 0 && ctx->tile_threads <= ND_Q_THREADS && ctx->V / ctx->tile_threads >= 2 * ctx->num_sms) {
+    if (ctx->tile_threads > 0 && ctx->tile_threads <= Q_THREADS && ctx->V / ctx->tile_threads >= 2 * ctx->num_sms) {
         threads = ctx->tile_threads;
         blocks = (unsigned)G.L0;
         for (int i = 0; i < 3; i++) { G.nt[i] = ctx->dims[i + 1] >> G.lb[i]; blocks *= (unsigned)G.nt[i]; }
