@@ -277,16 +277,16 @@ def run_b200(args):
         # (it synchronises for its small dense problems); eps then follows DESIGN.md R11.
         ctx.synchronize()
         t0 = time.perf_counter()
-        modes, nu, resid, st = ctx.lowmodes_compute(l, M_KERNEL, tol=args.eig_tol, maxit=60, lextra=max(8, l // 4),
-                                                    degree=args.eig_degree)
+        modes, nu, resid, st = ctx.lowmodes_compute(max(1, l - l // 8), M_KERNEL, tol=args.eig_tol, maxit=60, lextra=max(8, l // 4),
+                                                    degree=args.eig_degree, l_max=l + l // 8, stop="bound")
+        l = st["l_chosen"]
         ctx.synchronize()
-        eig = {"seconds": time.perf_counter() - t0, "l": l, "tol_Q2_residual": args.eig_tol, "converged": st["converged"],
+        eig = {"seconds": time.perf_counter() - t0, "l": l, "tol_bound_2_10": args.eig_tol, "converged": st["converged"],
                "outer_iterations": st["iterations"], "q_stencils": st["stencils"], "max_residue_Q": float(resid.max()),
                "nu2_min": float((nu ** 2).min()), "nu2_max": float((nu ** 2).max())}
-        rest = np.sqrt(np.maximum(st["theta_rest"], 0.0))
-        kappa, bound, _ = nd.projector_error(nu, resid, np.concatenate([rest, -rest]))     # eq. 2.9-2.10
-        eig["kappa_pm"] = [float(kappa[0]), float(kappa[1])]
-        eig["projector_bound_pm"] = [float(b) if np.isfinite(b) else None for b in bound]
+        eig["l_chosen"] = l
+        eig["kappa_pm"] = [float(st["kappa"][0]), float(st["kappa"][1])]                 # eq. 2.9
+        eig["projector_bound_pm"] = [float(b) if np.isfinite(b) else None for b in st["bound"]]   # eq. 2.10
         args.eps = 0.99 * float((nu ** 2).max()) / qnorm ** 2
         c, delta = nd.cheb_coeffs(n, args.eps)
         ctx.set_sign_poly(c, args.eps, qnorm, M_KERNEL)
@@ -422,7 +422,7 @@ def main():
     ap.add_argument("--field", default="haar", choices=["haar", "smooth"], help="gauge field recipe (DESIGN.md section 4)")
     ap.add_argument("--field-eps", type=float, default=0.25, help="eps of U = exp(i eps H) for --field smooth")
     ap.add_argument("--eigensolve", action="store_true", help="low modes from nd_lowmodes_compute (timed), eps by R11")
-    ap.add_argument("--eig-tol", type=float, default=2e-4)
+    ap.add_argument("--eig-tol", type=float, default=1e-2, help="stop when the bound (2.10) on the projector error is below this")
     ap.add_argument("--eig-degree", type=int, default=80)
     ap.add_argument("--quick", action="store_true", help="time only the line's own Q-kernel variant")
     ap.add_argument("--no-cpu-baseline", action="store_true")

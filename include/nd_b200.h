@@ -156,19 +156,30 @@ ND_API int nd_solve_DNm_mixed(nd_ctx* ctx64, nd_ctx* ctx32, void* x, const void*
                               int* stats);
 
 /* --------------------------------------------------------------------------------------------- low modes
- * The l lowest eigenpairs of Q^2 followed by the Rayleigh-Ritz step of Q in their span
- * (PAPER.md:L81): on return u_out holds u_k (device SoA, l vectors), nu[k] the Ritz values of Q (ascending in
- * nu^2), resid[k] = ||(Q - nu_k) u_k|| (eq. 2.8).  `m` is the kernel mass.  work: (2*(l+lextra)+4) device spinors.
- * Method: Chebyshev-filtered subspace iteration on Q^2 + Rayleigh-Ritz (R13); stops when all l
- * residuals of Q^2 are <= tol or after maxit outer iterations (ND_ERR_NO_CONVERGENCE, results still filled).
- * stats (may be NULL): [0] outer iterations, [1] stencil applications. */
-ND_API int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, double m, double tol, int maxit,
-                        unsigned long long seed, void* u_out, double* nu, double* resid, double* theta_rest,
-                        void* work, long long* stats);
-/* theta_rest (may be NULL): the lextra Ritz values of Q^2 of the guard vectors from the last Rayleigh-Ritz step,
- * ascending - upper estimates of the next eigenvalues of Q^2 above the l returned ones (input of nd_projector_error).
- *
- * Error control of the projectors (host utility, no GPU; eq. 2.8-2.10): from the Ritz values nu[l],
+ * nd_lowmodes_compute: the low modes of Q with their error control (section 2.3): minimise the block
+ * Ritz functional of Q^2 (L79; method: Chebyshev-filtered subspace iteration, R13), Rayleigh-Ritz of Q (eq. 2.7,
+ * L81) in the WHOLE block of k = l_max + lguard vectors, Ritz pairs sorted by |nu|, residues rho_j = ||(Q - nu_j) u_j||
+ * (eq. 2.8) for every j < k, and the number of projected modes chosen dynamically (L110; R17): l' in
+ * [l_min, l_max] at the largest gap |nu_{l'+1}| - |nu_{l'}|  (l_min == l_max fixes it).  d_k (L90) is estimated from the
+ * guard values |nu_j|, j >= l', taken with both signs, and the projected values of the opposite sign; kappa_+- by eq. 2.9,
+ * bound by eq. 2.10.  The iteration stops when (L110 "stopped when the desired level of precision is reached")
+ *     stop_rule 0:  rho_k <= tol for all k < l'           stop_rule 1:  max(bound_+, bound_-) <= tol
+ * or after maxit outer iterations (ND_ERR_NO_CONVERGENCE; all outputs are still filled with the last iterate).
+ *   m        kernel mass;  degree: Chebyshev filter degree per outer iteration;  seed: start vectors (nd_gaussian)
+ *   u_out    [out, device] l_max spinors; the first *l_chosen are the u_k of eq. 2.7, ascending in |nu|
+ *   nu,resid [out, host]   k values each: the whole block's Ritz values of Q and residues, ascending in |nu|
+ *                          (entries >= *l_chosen belong to the guard vectors)
+ *   kappa, bound [out, host, may be NULL] (kappa_+, kappa_-) and the two bounds (2.10); +inf where undefined
+ *   work     [device] nd_lowmodes_work_spinors(l_max, lguard) = 3k + 2 spinors
+ *   stats    (may be NULL) [0] outer iterations, [1] stencil applications */
+ND_API int nd_lowmodes_compute(nd_ctx* ctx, int l_min, int l_max, int lguard, int degree, double m, int stop_rule, double tol,
+                               int maxit, unsigned long long seed, void* u_out, double* nu, double* resid, int* l_chosen,
+                               double kappa[2], double bound[2], void* work, long long* stats);
+ND_API size_t nd_lowmodes_work_spinors(int l_max, int lguard);
+/* The gap rule alone (host utility, no GPU; R17): abs_nu[k] ascending moduli of the block's Ritz values;
+ * *l = the cut in [l_min, l_max] (l_max < k) with the largest gap abs_nu[l] - abs_nu[l-1] (ties: smallest l), *gap = it. */
+ND_API int nd_choose_l(int k, const double* abs_nu, int l_min, int l_max, int* l, double* gap);
+/* Error control of the projectors (host utility, no GPU; eq. 2.8-2.10): from the Ritz values nu[l],
  * the residues rho[l] (eq. 2.8) and estimates rest[nrest] of the eigenvalues of Q outside the low-mode space, compute
  *   d_k      = distance of nu_k from {rest} and from the Ritz values of the opposite sign
  *   kappa[0] = kappa_+, kappa[1] = kappa_-,  kappa_+-^2 = sum_{+-nu_k > 0} rho_k^2 / d_k^2              (2.9)
@@ -189,7 +200,9 @@ ND_API int nd_heev(int k, const double* a, double* w, double* z);
  *   nd_gamma5:     y <- gamma5 x  (y may alias x)
  *   nd_block_dot:  out[2k..2k+1] = <v_k, x>, k < l   (one pass over x and the block; host result)
  *   nd_block_axpy: y <- y + sum_k a[k] v_k           (a = l complex numbers on the host)
- *   nd_gaussian:   fill x with Re, Im ~ N(0,1) from a counter-based generator (Philox-4x32-10 + Box-Muller) */
+ *   nd_gaussian:   fill x with Re, Im ~ N(0,1) from a counter-based generator (Philox-4x32-10 + Box-Muller)
+ *   nd_*_dev:      the same reductions with the result left in the caller's DEVICE memory (2l / 2 / 2 doubles, (re, im)
+ *                  pairs; nd_norm2_dev: im = 0), enqueued on the context's stream without any synchronisation */
 ND_API int nd_axpy(nd_ctx* ctx, const double a[2], const void* x, void* y);
 ND_API int nd_scale(nd_ctx* ctx, const double a[2], void* x);
 ND_API int nd_copy(nd_ctx* ctx, void* y, const void* x);
@@ -198,6 +211,9 @@ ND_API int nd_norm2(nd_ctx* ctx, const void* x, double* out);
 ND_API int nd_gamma5(nd_ctx* ctx, void* y, const void* x);
 ND_API int nd_block_dot(nd_ctx* ctx, int l, const void* v, const void* x, double* out2l);
 ND_API int nd_block_axpy(nd_ctx* ctx, int l, const double* a2l, const void* v, void* y);
+ND_API int nd_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out2l);
+ND_API int nd_dot_dev(nd_ctx* ctx, const void* x, const void* y, double* d_out2);
+ND_API int nd_norm2_dev(nd_ctx* ctx, const void* x, double* d_out2);
 ND_API int nd_gaussian(nd_ctx* ctx, void* x, unsigned long long seed);
 
 #ifdef __cplusplus

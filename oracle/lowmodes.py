@@ -110,8 +110,8 @@ def projector_bound(kappa):
 def choose_l(abs_nu, l_min, l_max):
     """"The number of low modes included in the projector will be determined dynamically in such a way that the
     spectral distance from the other modes is not accidentally small".  Reading (R17): given
-    the moduli |nu_1| <= |nu_2| <= ... of the Ritz values of Q in the block (projected candidates AND guard vectors),
-    the cut l' in [l_min, l_max] is put at the LARGEST gap |nu_{l'+1}| - |nu_{l'}|; ties go to the smallest l'.
+    the ascending moduli a_1 <= a_2 <= ... of the Ritz values of Q in the block (projected candidates AND guard vectors),
+    the cut l' in [l_min, l_max] is put at the LARGEST gap a_{l'+1} - a_{l'}; ties go to the smallest l'.
     Needs len(abs_nu) >= l_max + 1 (at least one value beyond the last candidate)."""
     a = np.asarray(abs_nu, dtype=np.float64)
     assert np.all(np.diff(a) >= 0) and 1 <= l_min <= l_max < len(a)
@@ -124,13 +124,16 @@ def choose_l(abs_nu, l_min, l_max):
 
 
 def error_control(nu_block, rho_block, l_min, l_max):
-    """The whole error control of PAPER.md:L86-110 on a block of Ritz pairs of Q sorted by |nu| (eq. 2.8 residues
-    rho given): choose l' by `choose_l`; d_k (L90) from the Ritz values outside the cut - the guard values |nu_j|,
-    j >= l', taken with BOTH signs because a poorly converged guard vector does not fix its sign - and from the
-    projected values of the opposite sign; kappa_+- (2.9); bound (2.10).  Returns dict(l, gap, d, kappa, bound)."""
+    """The whole error control of PAPER.md:L86-110 on a block of Ritz pairs (nu_j, u_j) of Q with their residues rho_j
+    (eq. 2.8), ordered by the modulus estimate a_j = ||Q u_j|| = sqrt(nu_j^2 + rho_j^2) - for a converged pair a_j = |nu_j|;
+    a spurious small Ritz value of the indefinite Q comes with a large residue and sorts to the end (R17).
+    l' by `choose_l` on the a_j (made monotone by a running maximum: only unconverged guard pairs are affected); d_k (L90)
+    from the moduli outside the cut, a_j for j >= l', taken with BOTH signs because a poorly converged guard vector does
+    not fix its sign, and from the projected values of the opposite sign; kappa_+- (2.9); bound (2.10).
+    Returns dict(l, gap, d, kappa, bound)."""
     nu = np.asarray(nu_block, dtype=np.float64)
     rho = np.asarray(rho_block, dtype=np.float64)
-    a = np.abs(nu)
+    a = np.maximum.accumulate(np.sqrt(nu * nu + rho * rho))
     l, gap = choose_l(a, l_min, l_max)
     rest = np.concatenate([a[l:], -a[l:]])
     d = distances_d(nu[:l], rest)

@@ -53,8 +53,10 @@ SIGNATURES = {
     "nd_solve_DNm_mixed": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_dbl, _c_dbl, _c_int, _c_int, _c_vp, _c_vp, _pd,
                                     ctypes.POINTER(_c_int)]),
     "nd_convert_spinor": (_c_int, [_c_vp, _c_vp, _c_int, _c_vp, _c_int]),
-    "nd_lowmodes_compute": (_c_int, [_c_vp, _c_int, _c_int, _c_int, _c_dbl, _c_dbl, _c_int, _c_ull, _c_vp, _pd, _pd, _pd,
-                                     _c_vp, ctypes.POINTER(_c_ll)]),
+    "nd_lowmodes_compute": (_c_int, [_c_vp, _c_int, _c_int, _c_int, _c_int, _c_dbl, _c_int, _c_dbl, _c_int, _c_ull, _c_vp, _pd, _pd,
+                                     ctypes.POINTER(_c_int), _pd, _pd, _c_vp, ctypes.POINTER(_c_ll)]),
+    "nd_lowmodes_work_spinors": (_c_sz, [_c_int, _c_int]),
+    "nd_choose_l": (_c_int, [_c_int, _pd, _c_int, _c_int, ctypes.POINTER(_c_int), _pd]),
     "nd_projector_error": (_c_int, [_c_int, _pd, _pd, _c_int, _pd, _pd, _pd, _pd]),
     "nd_heev": (_c_int, [_c_int, _pd, _pd, _pd]),
     "nd_axpy": (_c_int, [_c_vp, _pd, _c_vp, _c_vp]),
@@ -65,6 +67,9 @@ SIGNATURES = {
     "nd_gamma5": (_c_int, [_c_vp, _c_vp, _c_vp]),
     "nd_block_dot": (_c_int, [_c_vp, _c_int, _c_vp, _c_vp, _pd]),
     "nd_block_axpy": (_c_int, [_c_vp, _c_int, _pd, _c_vp, _c_vp]),
+    "nd_block_dot_dev": (_c_int, [_c_vp, _c_int, _c_vp, _c_vp, _c_vp]),
+    "nd_dot_dev": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp]),
+    "nd_norm2_dev": (_c_int, [_c_vp, _c_vp, _c_vp]),
     "nd_gaussian": (_c_int, [_c_vp, _c_vp, _c_ull]),
 }
 
@@ -136,6 +141,17 @@ def projector_error(nu, rho, rest):
     if rc != ND_OK:
         raise NDError(rc, "nd_projector_error")
     return kappa, bound, d
+
+
+def choose_l(abs_nu, l_min, l_max):
+    """nd_choose_l: (l', gap) of the gap rule (R17) - host utility, needs no GPU."""
+    lib = load_library()
+    a = np.ascontiguousarray(abs_nu, dtype=np.float64)
+    l, gap = ctypes.c_int(0), ctypes.c_double(0.0)
+    rc = lib.nd_choose_l(len(a), a.ctypes.data_as(_pd), int(l_min), int(l_max), ctypes.byref(l), ctypes.byref(gap))
+    if rc != ND_OK:
+        raise NDError(rc, "nd_choose_l")
+    return l.value, gap.value
 
 
 def _ptr(x):
@@ -333,21 +349,30 @@ class Context:
     def convert_spinor(self, dst, dst_prec, src, src_prec):
         self._chk(self.lib.nd_convert_spinor(self._h, dst.data_ptr(), int(dst_prec), src.data_ptr(), int(src_prec)))
 
-    def lowmodes_compute(self, l, m, tol=1e-8, maxit=50, lextra=8, degree=40, seed=7):
-        """-> (u [l, 24V] device tensor, nu[l], resid[l], stats dict)."""
-        u = self.new_spinor(l)
-        work = self.new_spinor(2 * (l + lextra) + 4)
-        nu = np.zeros(l)
-        resid = np.zeros(l)
+    def lowmodes_compute(self, l, m, tol=1e-8, maxit=50, lextra=8, degree=40, seed=7, l_max=None, stop="residue"):
+        """nd_lowmodes_compute with l_min = l, l_max (default l: fixed number of modes), lguard = lextra guard vectors;
+        stop = "residue" (rho_k <= tol) or "bound" (bound (2.10) <= tol).
+        -> (u [l', 24V] device tensor, nu[l'], resid[l'], stats dict)."""
+        l_max = int(l if l_max is None else l_max)
+        k = l_max + int(lextra)
+        u = self.new_spinor(l_max)
+        work = self.new_spinor(int(self.lib.nd_lowmodes_work_spinors(l_max, int(lextra))))
+        nu, resid = np.zeros(k), np.zeros(k)
+        kappa, bound = np.zeros(2), np.zeros(2)
+        lc = ctypes.c_int(0)
         stats = (_c_ll * 2)()
-        rest = np.zeros(max(int(lextra), 1))
-        rc = self.lib.nd_lowmodes_compute(self._h, int(l), int(lextra), int(degree), float(m), float(tol), int(maxit),
+        rule = {"residue": 0, "bound": 1}[stop]
+        rc = self.lib.nd_lowmodes_compute(self._h, int(l), l_max, int(lextra), int(degree), float(m), rule, float(tol), int(maxit),
                                           int(seed), u.data_ptr(), nu.ctypes.data_as(_pd), resid.ctypes.data_as(_pd),
-                                          rest.ctypes.data_as(_pd), work.data_ptr(), stats)
+                                          ctypes.byref(lc), kappa.ctypes.data_as(_pd), bound.ctypes.data_as(_pd),
+                                          work.data_ptr(), stats)
         if rc not in (ND_OK, -6):
             self._chk(rc)
-        return u, nu, resid, dict(iterations=int(stats[0]), stencils=int(stats[1]), converged=(rc == ND_OK),
-                                  theta_rest=rest[:int(lextra)])
+        lp = lc.value
+        return u[:lp], nu[:lp].copy(), resid[:lp].copy(), dict(
+            iterations=int(stats[0]), stencils=int(stats[1]), converged=(rc == ND_OK), l_chosen=lp, kappa=kappa, bound=bound,
+            nu_block=nu, rho_block=resid, nu_guard=nu[lp:].copy(), theta_rest=np.sort(nu[lp:] ** 2),
+            message=(self.lib.nd_last_error(self._h).decode() if rc != ND_OK else ""))
 
     # -- BLAS-1
     def axpy(self, a, x, y):
@@ -377,6 +402,16 @@ class Context:
         out = np.zeros(2 * l)
         self._chk(self.lib.nd_block_dot(self._h, l, v.data_ptr(), x.data_ptr(), out.ctypes.data_as(_pd)))
         return out[0::2] + 1j * out[1::2]
+
+    def block_dot_dev(self, v, x, out):
+        """out: device float64 tensor of 2l entries, (re, im) pairs; no synchronisation."""
+        self._chk(self.lib.nd_block_dot_dev(self._h, v.shape[0], v.data_ptr(), x.data_ptr(), out.data_ptr()))
+
+    def dot_dev(self, x, y, out):
+        self._chk(self.lib.nd_dot_dev(self._h, x.data_ptr(), y.data_ptr(), out.data_ptr()))
+
+    def norm2_dev(self, x, out):
+        self._chk(self.lib.nd_norm2_dev(self._h, x.data_ptr(), out.data_ptr()))
 
     def block_axpy(self, a, v, y):
         a = np.asarray(a, dtype=np.complex128)

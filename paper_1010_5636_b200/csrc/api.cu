@@ -75,6 +75,8 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->num_sms = 148;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     ctx->err[0] = 0;
+    ctx->tile_ctas_per_sm[0] = ctx->tile_ctas_per_sm[1] = 0;
+    ctx->use_tile_kernel = ndi_tile_supported(ctx);
     // fp32 recon 18 is stored as 9 float2, everything else in 128-bit words: bytes = 4 * recon * V * prec/8
     ctx->gauge_bytes = (size_t)4 * recon * ctx->V * (prec / 8);
     cudaError_t e = cudaMalloc(&ctx->gauge, ctx->gauge_bytes);

@@ -269,6 +269,41 @@ __global__ void __launch_bounds__(RED_THREADS) block_rotate_kernel(typename Prec
     }
 }
 
+// ---------------------------------------------------------------------------------------- block residual
+// partial[j][block] = sum over the block's sites of |y_j - nu_j x_j|^2   (blockIdx.y = j): the residues of eq. 2.8 for a
+// whole block of Ritz pairs in one launch (differences formed in fp64)
+template <typename T>
+__global__ void __launch_bounds__(RED_THREADS) block_resid_kernel(double* __restrict__ partial, const double* __restrict__ nu,
+                                                                  const typename Prec<T>::Vec* __restrict__ x,
+                                                                  const typename Prec<T>::Vec* __restrict__ y, long long V) {
+    __shared__ double sm[RED_WARPS];
+    const int j = blockIdx.y;
+    const double nj = nu[j];
+    const typename Prec<T>::Vec* xj = x + (long long)j * Prec<T>::NV * V;
+    const typename Prec<T>::Vec* yj = y + (long long)j * Prec<T>::NV * V;
+    double acc = 0.0;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < V; s += (long long)gridDim.x * blockDim.x) {
+        cx<T> a[12], b[12];
+        load_site<T>(xj, V, s, a);
+        load_site<T>(yj, V, s, b);
+#pragma unroll
+        for (int i = 0; i < 12; i++) {
+            const double dr = (double)b[i].re - nj * (double)a[i].re, di = (double)b[i].im - nj * (double)a[i].im;
+            acc = fma(dr, dr, acc);
+            acc = fma(di, di, acc);
+        }
+    }
+    acc = warp_sum(acc);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < RED_WARPS; w++) t += sm[w];
+        partial[(long long)j * gridDim.x + blockIdx.x] = t;
+    }
+}
+
 // --------------------------------------------------------------------------------------------- gaussian
 __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0, unsigned k1,
                                               unsigned (&out)[4]) {
@@ -370,6 +405,24 @@ int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, 
     return ND_OK;
 }
 
+// rho_j = ||y_j - nu_j x_j||, j < k (host nu in, host rho out; synchronises)
+int ndi_block_resid(nd_ctx* ctx, int k, const void* x, const void* y, const double* nu, double* rho) {
+    ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < k; i++) ctx->h_result[i] = nu[i];
+    ND_CUDA(ctx, cudaMemcpyAsync(ctx->d_coef, ctx->h_result, (size_t)k * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    long long bx = (ctx->V + 8 * RED_THREADS - 1) / (8 * RED_THREADS);
+    if (bx > ctx->num_sms) bx = ctx->num_sms;
+    const dim3 grid((unsigned)bx, (unsigned)k, 1);
+    if (ctx->prec == 32) block_resid_kernel<float><<<grid, RED_THREADS, 0, ctx->stream>>>(ctx->d_partial, ctx->d_coef, (const float4*)x, (const float4*)y, ctx->V);
+    else block_resid_kernel<double><<<grid, RED_THREADS, 0, ctx->stream>>>(ctx->d_partial, ctx->d_coef, (const double2*)x, (const double2*)y, ctx->V);
+    ND_LAUNCHED(ctx);
+    reduce_partials_kernel<<<k, RED_THREADS, 0, ctx->stream>>>(ctx->d_result, ctx->d_partial, (int)bx);
+    ND_LAUNCHED(ctx);
+    int rc = ndi_read_result(ctx, ctx->d_result, rho, k);
+    for (int i = 0; i < k && rc == ND_OK; i++) rho[i] = sqrt(rho[i] > 0.0 ? rho[i] : 0.0);
+    return rc;
+}
+
 // G[k][j] = <v_k, x_j>, k < l, j < nx, into d_out[(j*l + k)*2 + {re, im}] (device); x_j at x + j*spinor_bytes
 int ndi_block_gram_dev(nd_ctx* ctx, int l, const void* v, int nx, const void* x, double* d_out) {
     const size_t sb = nd_spinor_bytes(ctx);
@@ -451,6 +504,15 @@ extern "C" int nd_block_dot(nd_ctx* ctx, int l, const void* v, const void* x, do
     return ndi_read_result(ctx, ctx->d_result, out2l, 2 * l);
 }
 extern "C" int nd_dot(nd_ctx* ctx, const void* x, const void* y, double out[2]) { return nd_block_dot(ctx, 1, x, y, out); }
+// results left in the caller's DEVICE memory, no synchronisation (SURVEY 8(b) `_dev` variants)
+extern "C" int nd_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out2l) {
+    ND_ENTER(ctx);
+    if (l < 1 || l > ND_MAX_BLOCK_L || !v || !x || !d_out2l) return nd_fail(ctx, ND_ERR_BAD_ARG, "block_dot_dev: bad argument (1 <= l <= %d)", ND_MAX_BLOCK_L);
+    return ndi_block_dot_dev(ctx, l, v, x, d_out2l);
+}
+extern "C" int nd_dot_dev(nd_ctx* ctx, const void* x, const void* y, double* d_out2) { return nd_block_dot_dev(ctx, 1, x, y, d_out2); }
+extern "C" int nd_norm2_dev(nd_ctx* ctx, const void* x, double* d_out2) { return nd_block_dot_dev(ctx, 1, x, x, d_out2); }
+
 extern "C" int nd_norm2(nd_ctx* ctx, const void* x, double* out) {
     double t[2];
     int rc = nd_block_dot(ctx, 1, x, x, t);

@@ -1,21 +1,24 @@
-// lowmodes.cu - the l lowest eigenpairs of Q^2 and the Rayleigh-Ritz step of Q in their span (PAPER.md:L79-88,
-// section 2.3, eq. 2.7-2.8).
+// lowmodes.cu - the low modes of Q and the error control of their projectors (section 2.3, eq. 2.7-2.10).
 //
 // PAPER.md:L79 says only that the low modes are found "by minimizing the Ritz functional of Q^2" (ref. [13]); no steps
-// are given.  DESIGN.md reading R13: any method delivering ||Q^2 x - theta x|| <= tol with orthonormal x.  Built here:
-// Chebyshev-filtered block subspace iteration, which minimises the block Ritz functional tr(X^dagger Q^2 X) over
-// orthonormal blocks X and is made of exactly the kernels D_N uses (plain stencil, stencil with the fused three-term
-// epilogue, block dot, grouped Gram / rotation kernels):
+// are given.  DESIGN.md reading R13: any method that delivers small residues; R17: the dynamic choice of l (L110).
+// Built here: Chebyshev-filtered block subspace iteration, which minimises the block Ritz functional
+// tr(X^dagger Q^2 X) over orthonormal blocks X and is made of exactly the kernels D_N uses (plain stencil, stencil with
+// the fused three-term epilogue, grouped Gram / rotation kernels), with the Rayleigh-Ritz step of Q (eq. 2.7) done in
+// the WHOLE block so that +nu / -nu partners are never separated by the cut:
 //
-//   X = k = l + lextra Gaussian vectors, orthonormalised
-//   repeat:  X_j <- T_d((Q^2 - c)/e) X_j       [c-e, c+e] = [cut, qnorm^2] is damped, everything below cut amplified
-//            orthonormalise X  (Gram matrix, Hermitian eigendecomposition on the host, X <- X W Lambda^{-1/2}; repeated
-//                               when the Gram matrix is ill-conditioned)
-//            Rayleigh-Ritz of Q^2 in span X: H = X^dagger (Q^2 X), H = W Theta W^dagger, X <- X W
-//            residuals r_j = ||Q^2 x_j - theta_j x_j|| for j < l (computed explicitly), cut <- theta_{k-1};
-//            leading columns with r_j <= tol/2 are locked (not filtered again)
-//   until max_j r_j <= tol
-//   Rayleigh-Ritz of Q in the span of the l lowest x_j: M = X^dagger Q X -> (nu_k, u_k), rho_k = ||(Q - nu_k) u_k||   (2.7, 2.8)
+//   X = k = l_max + lguard Gaussian vectors, orthonormalised
+//   repeat:  X_j <- p_d(Q^2) X_j, p_d = the degree-d Chebyshev polynomial that is small on [cut, qnorm^2] and normalised
+//                                 to 1 at the lowest Ritz value (scaled three-term recurrence: no overflow in fp32);
+//                                 columns whose residue is already far below what the tolerance needs are locked
+//            orthonormalise X    (equilibrated Gram matrix, Hermitian eigendecomposition on the host,
+//                                 X <- X D^{-1/2} W Lambda^{-1/2}; repeated while the Gram matrix is ill-conditioned)
+//            Y = Q X;  H = Y^dagger Y (-> largest Ritz value of Q^2 in the block = next cut);
+//            M = X^dagger Y = W diag(nu) W^dagger: Rayleigh-Ritz of Q in the block (2.7); pairs ordered by
+//            a_j = ||Q u_j|| = sqrt(nu_j^2 + rho_j^2) (= |nu_j| once converged);  X <- X W
+//            Y = Q X;  rho_j = ||Y_j - nu_j X_j||  for every j                                        (2.8)
+//            cut l' in [l_min, l_max] at the largest gap of a_j (R17); d_k, kappa_+-, bound           (2.9, 2.10)
+//   until the stop rule holds:  rule 0: max_{k < l'} rho_k <= tol      rule 1: max(bound_+, bound_-) <= tol   (L110)
 //
 // Everything of size V runs on the GPU; the k x k Hermitian eigenproblems (k <= 256) run on the host in fp64 with a
 // cyclic Jacobi method (nd_heev, no LAPACK dependency).
@@ -43,11 +46,12 @@ extern "C" int nd_heev(int k, const double* a_in, double* w, double* z_out) {
     double scale = 0.0;
     for (auto& x : A) scale = std::max(scale, std::abs(x));
     if (scale == 0.0) scale = 1.0;
-    for (int sweep = 0; sweep < 60; sweep++) {
+    bool done = false;
+    for (int sweep = 0; sweep < 60 && !done; sweep++) {
         double off = 0.0;
         for (int p = 0; p < k; p++)
             for (int q = p + 1; q < k; q++) off += std::norm(A[(size_t)p * k + q]);
-        if (std::sqrt(off) <= 1e-14 * scale * std::sqrt((double)k)) break;   // off-diagonal Frobenius norm at rounding level
+        if (std::sqrt(off) <= 1e-14 * scale * std::sqrt((double)k)) { done = true; break; }   // off-diagonal Frobenius norm at rounding level
         for (int p = 0; p < k; p++)
             for (int q = p + 1; q < k; q++) {
                 const zc apq = A[(size_t)p * k + q];
@@ -88,6 +92,13 @@ extern "C" int nd_heev(int k, const double* a_in, double* w, double* z_out) {
                 A[(size_t)q * k + q] = A[(size_t)q * k + q].real();
             }
     }
+    if (!done) {
+        // the sweep limit was hit: accept only if the last sweep did bring the off-diagonal part down to rounding level
+        double off = 0.0;
+        for (int p = 0; p < k; p++)
+            for (int q = p + 1; q < k; q++) off += std::norm(A[(size_t)p * k + q]);
+        if (!(std::sqrt(off) <= 1e-12 * scale * std::sqrt((double)k))) return ND_ERR_NO_CONVERGENCE;
+    }
     std::vector<int> order(k);
     for (int i = 0; i < k; i++) order[i] = i;
     std::sort(order.begin(), order.end(), [&](int x, int y) { return A[(size_t)x * k + x].real() < A[(size_t)y * k + y].real(); });
@@ -123,6 +134,21 @@ extern "C" int nd_projector_error(int l, const double* nu, const double* rho, in
     return ND_OK;
 }
 
+extern "C" int nd_choose_l(int k, const double* abs_nu, int l_min, int l_max, int* l, double* gap) {
+    if (!abs_nu || !l || l_min < 1 || l_max < l_min || l_max >= k) return ND_ERR_BAD_ARG;
+    for (int i = 1; i < k; i++)
+        if (!(abs_nu[i] >= abs_nu[i - 1]) || !(abs_nu[i - 1] >= 0.0)) return ND_ERR_BAD_ARG;   // ascending moduli (NaN fails)
+    int best = l_min;
+    double best_gap = -1.0;
+    for (int c = l_min; c <= l_max; c++) {
+        const double g = abs_nu[c] - abs_nu[c - 1];
+        if (g > best_gap) { best = c; best_gap = g; }
+    }
+    *l = best;
+    if (gap) *gap = best_gap;
+    return ND_OK;
+}
+
 namespace {
 
 struct Solver {
@@ -130,7 +156,7 @@ struct Solver {
     size_t sb;
     int k;
     double m;
-    char *X, *Y, *s0, *s1, *s2;
+    char *X, *Y, *Z, *s0, *s1;
     double* d_mat;   // 2 k^2 doubles on the device
     std::vector<double> h_mat;
     long long stencils;
@@ -173,92 +199,108 @@ struct Solver {
         ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));   // `col` is pageable and dies with this frame
         return ndi_block_rotate_dev(ctx, ns, d_mat, src, nd, dst);
     }
-    // X <- X W Lambda^{-1/2} with X^dagger X = W Lambda W^dagger (result back in X)
-    int orthonormalise(int reps) {
-        std::vector<double> w(k), z((size_t)2 * k * k);
-        for (int r = 0; r < reps; r++) {
+    // X <- X D^{-1/2} W Lambda^{-1/2} with D = diag(G), D^{-1/2} G D^{-1/2} = W Lambda W^dagger, G = X^dagger X.
+    // The column scaling takes the grading of the filtered block (column norms differ by orders of magnitude) out of the
+    // eigenproblem; passes are repeated while the equilibrated Gram matrix is ill-conditioned (the loss of orthogonality
+    // of one pass is ~ rounding * cond), and the result is refused if it does not get well-conditioned.
+    int orthonormalise() {
+        std::vector<double> w(k), z((size_t)2 * k * k), dscale(k);
+        const double cond_ok = (ctx->prec == 32) ? 30.0 : 1.0e6;
+        for (int pass = 0; pass < 5; pass++) {
             int rc = gram(X, k, X, k);
             if (rc != ND_OK) return rc;
+            for (int j = 0; j < k; j++) {
+                const double g = h_mat[2 * ((size_t)j * k + j)];
+                if (!(g > 0.0) || !std::isfinite(g)) return nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "lowmodes: block column %d has norm^2 %g", j, g);
+                dscale[j] = 1.0 / std::sqrt(g);
+            }
+            for (int i = 0; i < k; i++)
+                for (int j = 0; j < k; j++) {
+                    h_mat[2 * ((size_t)i * k + j)] *= dscale[i] * dscale[j];
+                    h_mat[2 * ((size_t)i * k + j) + 1] *= dscale[i] * dscale[j];
+                }
             rc = nd_heev(k, h_mat.data(), w.data(), z.data());
-            if (rc != ND_OK) return rc;
+            if (rc != ND_OK) return nd_fail(ctx, rc, "lowmodes: Jacobi eigen-solver did not converge on the Gram matrix");
+            if (!(w[0] > 0.0) || !std::isfinite(w[0])) return nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "lowmodes: block lost rank (Gram eigenvalue %g)", w[0]);
+            const double cond = w[k - 1] / w[0];
+            if (pass > 0 && cond < 1.0 + (ctx->prec == 32 ? 1e-4 : 1e-12)) return ND_OK;   // already orthonormal to rounding
             std::vector<zc> C((size_t)k * k);
             for (int j = 0; j < k; j++) {
-                if (!(w[j] > 0.0) || !std::isfinite(w[j])) return nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "lowmodes: block lost rank (Gram eigenvalue %g)", w[j]);
                 const double f = 1.0 / std::sqrt(w[j]);
-                for (int i = 0; i < k; i++) C[(size_t)i * k + j] = f * zc(z[2 * ((size_t)i * k + j)], z[2 * ((size_t)i * k + j) + 1]);
+                for (int i = 0; i < k; i++) C[(size_t)i * k + j] = dscale[i] * f * zc(z[2 * ((size_t)i * k + j)], z[2 * ((size_t)i * k + j) + 1]);
             }
-            rc = rotate(Y, k, X, k, C);
+            rc = rotate(Z, k, X, k, C);
             if (rc != ND_OK) return rc;
-            std::swap(X, Y);
-            // the loss of orthogonality of X W Lambda^{-1/2} is ~ rounding * cond(Gram): a second pass only when needed
-            if (w[k - 1] / w[0] < (ctx->prec == 32 ? 30.0 : 1.0e6)) break;
+            std::swap(X, Z);
+            if (cond < cond_ok) return ND_OK;
         }
-        return ND_OK;
+        return nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "lowmodes: the block does not orthonormalise (Gram matrix stays ill-conditioned)");
     }
-    // X_j <- T_d((Q^2 - c)/e) X_j, d even; t_{i+1} = (2/e)(Q^2 - c) t_i - t_{i-1}, the update folded into the 2nd stencil
-    // columns j < first are locked (their residual met the tolerance): they stay in the block for the orthonormalisation
-    // and the Rayleigh-Ritz step but are not filtered again
-    int filter(int d, double lo, double hi, int first) {
+    // X_j <- p_d(Q^2) X_j for j >= first: scaled Chebyshev recurrence on [lo, hi] (damped), normalised to 1 at `low`
+    //   sigma_1 = e/(low - c);  t_1 = (sigma_1/e)(Q^2 - c) t_0
+    //   sigma_{i+1} = 1/(2/sigma_1 - sigma_i);  t_{i+1} = (2 sigma_{i+1}/e)(Q^2 - c) t_i - sigma_i sigma_{i+1} t_{i-1}
+    // each step = one plain stencil + one stencil with the update in its epilogue (the Clenshaw step's kernel); d even
+    int filter(int d, double low, double lo, double hi, int first) {
         const double c = 0.5 * (hi + lo), e = 0.5 * (hi - lo);
+        const double sigma1 = e / (low - c);
         for (int j = first; j < k; j++) {
             char* P = x(j);   // t_{i-1}
             char* R = s0;     // t_i
             int rc = Q(s1, P);
             if (rc != ND_OK) return rc;
-            rc = Qepi(R, s1, 1.0 / e, -c / e, P, 0.0, nullptr);   // t_1
+            rc = Qepi(R, s1, sigma1 / e, -c * sigma1 / e, P, 0.0, nullptr);   // t_1
             if (rc != ND_OK) return rc;
+            double sigma = sigma1;
             for (int i = 1; i < d; i++) {
+                const double sn = 1.0 / (2.0 / sigma1 - sigma);
                 rc = Q(s1, R);
                 if (rc != ND_OK) return rc;
-                rc = Qepi(P, s1, 2.0 / e, -2.0 * c / e, R, -1.0, P);   // t_{i+1} over t_{i-1}
+                rc = Qepi(P, s1, 2.0 * sn / e, -2.0 * sn * c / e, R, -sigma * sn, P);   // t_{i+1} over t_{i-1}
                 if (rc != ND_OK) return rc;
                 std::swap(P, R);
+                sigma = sn;
             }
             // d even: t_d sits in x(j) again
         }
         return ND_OK;
     }
-    int norm(const void* v, double* out) {
-        int rc = ndi_block_dot_dev(ctx, 1, v, v, ctx->d_result);
-        if (rc != ND_OK) return rc;
-        double t[2];
-        rc = ndi_read_result(ctx, ctx->d_result, t, 2);
-        *out = std::sqrt(std::max(t[0], 0.0));
-        return rc;
-    }
 };
 
 }  // namespace
 
-extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, double m, double tol, int maxit,
-                                   unsigned long long seed, void* u_out, double* nu, double* resid, double* theta_rest,
-                                   void* work, long long* stats) {
+extern "C" size_t nd_lowmodes_work_spinors(int l_max, int lguard) { return (size_t)3 * (l_max + lguard) + 2; }
+
+extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l_min, int l_max, int lguard, int degree, double m, int stop_rule, double tol,
+                                   int maxit, unsigned long long seed, void* u_out, double* nu, double* resid, int* l_chosen,
+                                   double kappa[2], double bound[2], void* work, long long* stats) {
     if (!ctx) return ND_ERR_BAD_ARG;
-    if (l < 1 || lextra < 0 || l + lextra > ND_MAX_BLOCK_L || degree < 2 || maxit < 1 || !(tol > 0.0) || !u_out || !nu ||
-        !resid || !work)
-        return nd_fail(ctx, ND_ERR_BAD_ARG, "lowmodes_compute: bad argument (1 <= l, l + lextra <= %d, degree >= 2)", ND_MAX_BLOCK_L);
+    if (l_min < 1 || l_max < l_min || lguard < 1 || l_max + lguard > ND_MAX_BLOCK_L || degree < 2 || maxit < 1 || !(tol > 0.0) ||
+        (stop_rule != 0 && stop_rule != 1) || !u_out || !nu || !resid || !l_chosen || !work)
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "lowmodes_compute: bad argument (1 <= l_min <= l_max, lguard >= 1, l_max + lguard <= %d, degree >= 2)",
+                       ND_MAX_BLOCK_L);
     if (!ctx->gauge_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "lowmodes_compute: gauge field not set");
-    if (12 * ctx->V < l + lextra) return nd_fail(ctx, ND_ERR_BAD_ARG, "lowmodes_compute: block larger than the space");
+    if (12 * ctx->V < l_max + lguard) return nd_fail(ctx, ND_ERR_BAD_ARG, "lowmodes_compute: block larger than the space");
     ND_CUDA(ctx, cudaSetDevice(ctx->device));
     Solver S;
     S.ctx = ctx;
     S.sb = nd_spinor_bytes(ctx);
-    S.k = l + lextra;
+    S.k = l_max + lguard;
     S.m = m;
     S.stencils = 0;
     const int k = S.k;
     S.X = (char*)work;
     S.Y = S.X + (size_t)k * S.sb;
-    S.s0 = S.Y + (size_t)k * S.sb;
+    S.Z = S.Y + (size_t)k * S.sb;
+    S.s0 = S.Z + (size_t)k * S.sb;
     S.s1 = S.s0 + S.sb;
-    S.s2 = S.s1 + S.sb;
     S.d_mat = nullptr;
     ND_CUDA(ctx, cudaMalloc((void**)&S.d_mat, (size_t)2 * k * k * sizeof(double)));
     const int d = degree + (degree & 1);
     const double hi = (std::fabs(4.0 + m) + 4.0) * (std::fabs(4.0 + m) + 4.0);   // ||Q||^2 <= (|4+m|+4)^2 (R6)
-    int rc = ND_OK, it = 0;
+    int rc = ND_OK, it = 0, lp = l_min;
     bool converged = false;
-    std::vector<double> theta(k), z((size_t)2 * k * k), rq(l, 0.0);
+    std::vector<double> theta(k), z((size_t)2 * k * k), nuv(k), rho(k, 0.0), dk(k, 0.0), amod(k), tau(k), Hm;
+    double kap[2] = {INFINITY, INFINITY}, bnd[2] = {INFINITY, INFINITY};
     auto finish = [&](int code) {
         cudaFree(S.d_mat);
         if (stats) { stats[0] = it; stats[1] = S.stencils; }
@@ -268,80 +310,97 @@ extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l, int lextra, int degree, d
         rc = nd_gaussian(ctx, S.x(j), seed + (unsigned long long)j);
         if (rc != ND_OK) return finish(rc);
     }
-    rc = S.orthonormalise(2);
+    rc = S.orthonormalise();
     if (rc != ND_OK) return finish(rc);
-    double cut = -1.0;   // unknown before the first Rayleigh-Ritz step
+    double cut = -1.0, low = 0.0;   // unknown before the first Rayleigh-Ritz step
     int nlock = 0;
     for (it = 0; it <= maxit; it++) {
         if (it > 0) {
-            rc = S.filter(d, cut, hi, nlock);
-            if (rc != ND_OK) return finish(rc);
-            rc = S.orthonormalise(2);
+            rc = S.filter(d, low, cut, hi, nlock);
+            if (rc == ND_OK) rc = S.orthonormalise();
             if (rc != ND_OK) return finish(rc);
         }
-        // Rayleigh-Ritz of Q^2: Y = Q^2 X, H = X^dagger Y
+        // Y = Q X;  H = Y^dagger Y = X^dagger Q^2 X: its extreme eigenvalues are the extreme Ritz values of Q^2 in the block
+        for (int j = 0; j < k && rc == ND_OK; j++) rc = S.Q(S.y(j), S.x(j));
+        if (rc == ND_OK) rc = S.gram(S.Y, k, S.Y, k);
+        if (rc != ND_OK) return finish(rc);
+        Hm.assign(S.h_mat.begin(), S.h_mat.end());
+        rc = nd_heev(k, Hm.data(), theta.data(), z.data());
+        // Rayleigh-Ritz of Q in the whole block (eq. 2.7): M = X^dagger Q X = W diag(nu) W^dagger
+        if (rc == ND_OK) rc = S.gram(S.X, k, S.Y, k);
+        if (rc == ND_OK) rc = nd_heev(k, S.h_mat.data(), nuv.data(), z.data());
+        if (rc != ND_OK) return finish(rc == ND_ERR_NO_CONVERGENCE ? nd_fail(ctx, rc, "lowmodes: Jacobi eigen-solver did not converge") : rc);
+        // Order the Ritz pairs by the Rayleigh quotient of Q^2, a_j^2 = ||Q u_j||^2 = w_j^dagger H w_j (= nu_j^2 + rho_j^2):
+        // for a converged pair a_j = |nu_j|, while a spurious small Ritz value of the indefinite Q (a vector mixing +nu and
+        // -nu modes whose partner combination is not in the block yet) has a large residue and goes to the end (R17).
         for (int j = 0; j < k; j++) {
-            rc = S.Q(S.s1, S.x(j));
-            if (rc == ND_OK) rc = S.Q(S.y(j), S.s1);
-            if (rc != ND_OK) return finish(rc);
+            double t = 0.0;
+            for (int a = 0; a < k; a++) {
+                zc acc(0.0, 0.0);
+                for (int b = 0; b < k; b++)
+                    acc += zc(Hm[2 * ((size_t)a * k + b)], Hm[2 * ((size_t)a * k + b) + 1]) * zc(z[2 * ((size_t)b * k + j)], z[2 * ((size_t)b * k + j) + 1]);
+                t += (std::conj(zc(z[2 * ((size_t)a * k + j)], z[2 * ((size_t)a * k + j) + 1])) * acc).real();
+            }
+            tau[j] = t;
         }
-        rc = S.gram(S.X, k, S.Y, k);
-        if (rc == ND_OK) rc = nd_heev(k, S.h_mat.data(), theta.data(), z.data());
-        if (rc != ND_OK) return finish(rc);
+        std::vector<int> order(k);
+        for (int i = 0; i < k; i++) order[i] = i;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return tau[a] < tau[b]; });
         std::vector<zc> W((size_t)k * k);
-        for (size_t i = 0; i < W.size(); i++) W[i] = zc(z[2 * i], z[2 * i + 1]);
-        rc = S.rotate(S.Y, k, S.X, k, W);
-        if (rc != ND_OK) return finish(rc);
-        std::swap(S.X, S.Y);
-        // explicit residuals of the l lowest Ritz pairs
-        double worst = 0.0;
-        for (int j = 0; j < l; j++) {
-            rc = S.Q(S.s1, S.x(j));
-            if (rc == ND_OK) rc = S.Qepi(S.s0, S.s1, 1.0, -theta[j], S.x(j), 0.0, nullptr);
-            if (rc == ND_OK) rc = S.norm(S.s0, &rq[j]);
-            if (rc != ND_OK) return finish(rc);
-            worst = std::max(worst, rq[j]);
+        for (int j = 0; j < k; j++) {
+            nu[j] = nuv[order[j]];
+            for (int i = 0; i < k; i++) W[(size_t)i * k + j] = zc(z[2 * ((size_t)i * k + order[j])], z[2 * ((size_t)i * k + order[j]) + 1]);
         }
-        if (worst <= tol) { converged = true; break; }
-        nlock = 0;
-        while (nlock < l && rq[nlock] <= 0.5 * tol) nlock++;   // leading Ritz pairs already well inside the tolerance
-        // damp everything above the block's largest Ritz value next time (keep the interval non-degenerate)
-        cut = std::min(theta[k - 1], 0.5 * hi);
-        if (lextra == 0) cut = std::min(theta[k - 1] * 1.05 + 1e-3, 0.5 * hi);
-    }
-    if (it > maxit) it = maxit;
-    if (theta_rest)
-        for (int j = l; j < k; j++) theta_rest[j - l] = theta[j];
-    // Rayleigh-Ritz of Q in the span of the l lowest vectors (eq. 2.7): Y_j = Q X_j, M = X^dagger Y
-    for (int j = 0; j < l; j++) {
-        rc = S.Q(S.y(j), S.x(j));
+        rc = S.rotate(S.Z, k, S.X, k, W);
         if (rc != ND_OK) return finish(rc);
-    }
-    rc = S.gram(S.X, l, S.Y, l);
-    std::vector<double> nuv(l), zq((size_t)2 * l * l);
-    if (rc == ND_OK) rc = nd_heev(l, S.h_mat.data(), nuv.data(), zq.data());
-    if (rc != ND_OK) return finish(rc);
-    std::vector<int> order(l);
-    for (int i = 0; i < l; i++) order[i] = i;
-    std::sort(order.begin(), order.end(), [&](int a, int b) { return nuv[a] * nuv[a] < nuv[b] * nuv[b]; });
-    std::vector<zc> Wq((size_t)l * l);
-    for (int j = 0; j < l; j++) {
-        nu[j] = nuv[order[j]];
-        for (int i = 0; i < l; i++) Wq[(size_t)i * l + j] = zc(zq[2 * ((size_t)i * l + order[j])], zq[2 * ((size_t)i * l + order[j]) + 1]);
-    }
-    rc = S.rotate((char*)u_out, l, S.X, l, Wq);
-    if (rc != ND_OK) return finish(rc);
-    for (int j = 0; j < l; j++) {
-        char* uj = (char*)u_out + (size_t)j * S.sb;
-        rc = S.Qepi(S.s0, uj, 1.0, -nu[j], uj, 0.0, nullptr);   // (Q - nu_j) u_j   (eq. 2.8)
-        if (rc == ND_OK) rc = S.norm(S.s0, &resid[j]);
+        std::swap(S.X, S.Z);
+        // residues rho_j = ||(Q - nu_j) u_j|| of the whole block (eq. 2.8), Q u_j recomputed on the rotated vectors
+        for (int j = 0; j < k && rc == ND_OK; j++) rc = S.Q(S.y(j), S.x(j));
+        if (rc == ND_OK) rc = ndi_block_resid(ctx, k, S.X, S.Y, nu, rho.data());
         if (rc != ND_OK) return finish(rc);
-    }
-    ND_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    if (!converged) {
+        for (int j = 0; j < k; j++) {
+            resid[j] = rho[j];
+            amod[j] = std::sqrt(nu[j] * nu[j] + rho[j] * rho[j]);
+        }
+        // the measured residues replace the small-matrix estimate; keep the list ascending for the gap rule (changes
+        // nothing for converged pairs, clamps the noise of unconverged guard pairs)
+        for (int j = 1; j < k; j++) amod[j] = std::max(amod[j], amod[j - 1]);
+        // error control: the cut, d_k from the guard moduli (both signs) and the opposite-sign values
+        rc = nd_choose_l(k, amod.data(), l_min, l_max, &lp, nullptr);
+        if (rc != ND_OK) return finish(nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "lowmodes: Ritz values not finite"));
+        bool signs_ok = true;
+        for (int j = 0; j < lp; j++) signs_ok = signs_ok && nu[j] != 0.0;
+        if (signs_ok) {
+            std::vector<double> rest((size_t)2 * (k - lp));
+            for (int j = lp; j < k; j++) { rest[2 * (j - lp)] = amod[j]; rest[2 * (j - lp) + 1] = -amod[j]; }
+            nd_projector_error(lp, nu, rho.data(), (int)rest.size(), rest.data(), kap, bnd, dk.data());
+        } else {
+            kap[0] = kap[1] = bnd[0] = bnd[1] = INFINITY;
+        }
         double worst = 0.0;
-        for (int j = 0; j < l; j++) worst = std::max(worst, rq[j]);
-        nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "lowmodes_compute: max residual of Q^2 %.3e > tol %.3e after %d iterations", worst, tol, it);
+        for (int j = 0; j < lp; j++) worst = std::max(worst, rho[j]);
+        converged = (stop_rule == 0) ? (worst <= tol) : (std::max(bnd[0], bnd[1]) <= tol);
+        if (converged || it == maxit) break;
+        // lock the leading columns whose residue is already far below what the stop rule needs from them
+        nlock = 0;
+        while (nlock < lp) {
+            const double need = (stop_rule == 0) ? 0.5 * tol : 0.25 * tol * dk[nlock] / std::sqrt((double)l_max);
+            if (!(rho[nlock] <= need)) break;
+            nlock++;
+        }
+        // damp everything above the block's largest Ritz value of Q^2 next time, normalise at its lowest one
+        cut = std::min(theta[k - 1], 0.5 * hi);
+        low = std::max(0.0, std::min(theta[0], 0.5 * cut));
+    }
+    *l_chosen = lp;
+    if (kappa) { kappa[0] = kap[0]; kappa[1] = kap[1]; }
+    if (bound) { bound[0] = bnd[0]; bound[1] = bnd[1]; }
+    rc = nd_cuda_check(ctx, cudaMemcpyAsync(u_out, S.X, (size_t)l_max * S.sb, cudaMemcpyDeviceToDevice, ctx->stream), "lowmodes copy-out");
+    if (rc == ND_OK) rc = nd_cuda_check(ctx, cudaStreamSynchronize(ctx->stream), "lowmodes sync");
+    if (rc != ND_OK) return finish(rc);
+    if (!converged) {
+        nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "lowmodes_compute: after %d iterations l' = %d, max residue %.3e, kappa = (%.3e, %.3e), stop rule %d not met (tol %.3e)",
+                it, lp, *std::max_element(rho.begin(), rho.begin() + lp), kap[0], kap[1], stop_rule, tol);
         return finish(ND_ERR_NO_CONVERGENCE);
     }
     return finish(ND_OK);

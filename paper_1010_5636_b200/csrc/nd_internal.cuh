@@ -59,6 +59,8 @@ struct nd_ctx {
     int hop_max_sites;  // lattices below this volume use the hop-parallel stencil (wilson.cu)
     int tile_lb[3];     // stencil CTA tile: log2 extents along x1, x2, x3
     int tile_threads;   // sites per tile (0: linear mapping)
+    bool use_tile_kernel;       // the tiled marching stencil (wilson_tile.cu) takes this lattice
+    int tile_ctas_per_sm[2];    // its resident CTAs per SM (plain / fused epilogue), 0 = not queried yet
     char err[512];
 };
 
@@ -150,6 +152,9 @@ __device__ __forceinline__ void cx_to_words(const cx<double> (&c)[12], double2 (
 // ---------------------------------------------------------------------------- internal entry points (per TU)
 int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
                 double s2, const void* v2, double s3, const void* v3);
+bool ndi_tile_supported(const nd_ctx* ctx);
+int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
+                     const void* v2, double s3, const void* v3);
 int ndi_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out);   // d_out: 2l doubles (device)
 int ndi_block_dot2_dev(nd_ctx* ctx, int l, const void* v, const void* x0, const void* x1, double* d_out);  // 4l doubles
 int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pa,
@@ -157,6 +162,7 @@ int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, 
 int ndi_apply_DNm(nd_ctx* ctx, void* out, const void* in, double pa, double pb, void* work, int use_graph);
 int ndi_block_gram_dev(nd_ctx* ctx, int l, const void* v, int nx, const void* x, double* d_out);      // d_out[(j*l+k)*2+c]
 int ndi_block_rotate_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, int ny, void* y);  // coef[(j*l+i)*2+c]
+int ndi_block_resid(nd_ctx* ctx, int k, const void* x, const void* y, const double* nu, double* rho);   // rho_j = ||y_j - nu_j x_j||
 int ndi_read_result(nd_ctx* ctx, const double* d_src, double* h_dst, int n);              // sync copy to host
 int ndi_drop_graphs(nd_ctx* ctx);
 constexpr int ND_RESULT_DOUBLES = 4 * ND_MAX_BLOCK_L;

@@ -10,9 +10,12 @@ template <typename T> __device__ __forceinline__ void unpack_reals(const float2&
 template <typename T> __device__ __forceinline__ void unpack_reals(const float4& v, T* r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
 template <typename T> __device__ __forceinline__ void unpack_reals(const double2& v, T* r) { r[0] = v.x; r[1] = v.y; }
 
-__device__ __forceinline__ float nd_sqrt(float x) { return __fsqrt_rn(x); }
-// correctly rounded reciprocals (rcp.rn): a handful of instructions instead of the general division routine
-__device__ __forceinline__ float nd_rcp(float x) { return __frcp_rn(x); }
+// fp32: the special-function unit's sqrt / reciprocal (one MUFU instruction each, <= 1-2 ulp) - the 8-parameter form is bound by
+// its reconstruction arithmetic, not by memory, and its rounding error is dominated by the 1/N amplification (R8),
+// not by the last ulp of these two; the arguments are never denormal (N >= 1e-6 is enforced by nd_set_gauge, 1 + q^2 >= 1).
+__device__ __forceinline__ float nd_sqrt(float x) { float r; asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float nd_rcp(float x) { float r; asm("rcp.approx.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+// fp64: correctly rounded reciprocal (rcp.rn): a handful of instructions instead of the general division routine
 __device__ __forceinline__ double nd_rcp(double x) { return __drcp_rn(x); }
 __device__ __forceinline__ double nd_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ float nd_max0(float x) { return fmaxf(x, 0.f); }

@@ -1,0 +1,504 @@
+// wilson_tile.cu - the Wilson-Dirac stencil Q = gamma5 D_W (eq. 2.1-2.2) as a tiled, marching kernel with
+// neighbour exchange through shared memory (BASELINE.json north_star subsystem 2: "stages neighbour halos in shared memory").
+//
+// Why: the site-per-thread kernel (wilson.cu) moves its compulsory bytes through HBM exactly once, but pulls every
+// neighbour spinor and every backward link through the L2 -> SM fabric again (822 B/site in fp32 for 384 B compulsory,
+// profiles/r01_q_kernel_ncu_full.md) and sits at that fabric's limit, not at the HBM roofline.  Here
+//   * a CTA owns a tile of B1 x B2 x L3 sites of one time-slice (x3 in full, so the warp runs along whole x3 rows) and
+//     MARCHES along x0 over a segment of time-slices; a thread owns one (x1, x2, x3) column;
+//   * every thread loads ITS OWN spinor and ITS OWN four links, once, fully coalesced (288 B/site in fp32 = the compulsory
+//     input traffic), reconstructs each link once, and SENDS to its neighbours, through shared memory, what they need:
+//         h-_mu(x) = (1 - gamma_mu) phi(x)                 to x - mu^  (which multiplies by its own U_mu(x - mu^))
+//         w_mu(x)  = U_mu(x)^dagger (1 + gamma_mu) phi(x)   to x + mu^  (its complete backward hop)
+//     as half-spinors (12 reals) - so no thread ever loads a neighbour's link, and every link is rebuilt by its owner only;
+//   * the x3 neighbours are in the same warp: exchanged with shuffles; the x0 neighbours are the thread's own column:
+//     phi(t+1) is prefetched into registers and the backward time hop w_0 is carried from the previous slice;
+//   * only tile-face sites read neighbour data from global memory (the halo: phi for a forward face, phi and the one link
+//     for a backward face) and put the resulting half-spinor into their own receive slot, so the receive phase is uniform;
+//   * the links of the NEXT slice travel by cp.async straight into a private shared-memory slot of the thread that owns
+//     them while the current slice is computed: a whole slice of link data per CTA is in flight without holding registers;
+//   * x1 and x2 use separate exchange buffers in turn (send x1, barrier, receive x1, send x2, barrier, receive x2): two
+//     __syncthreads per time-slice and no buffer is ever written while it may still be read.
+// L2 -> SM traffic per site (fp32, recon 12, tile 2 x 4 x 32): 288 own + 96 store + 180 halo = 564 B; tile 4 x 4 x 32: 504 B.
+#include "nd_dirac.cuh"
+
+namespace {
+
+struct TileGeom {
+    int L0, L1, L2;
+    long long V, S0;
+    int bc;
+    int nt2, ntile;          // tiles along x2, tiles per time-slice
+    int seg_base, seg_rem;   // nseg segments of time-slices: the first seg_rem have seg_base + 1 slices, the rest seg_base
+};
+
+template <typename T> struct HalfWords { static constexpr int NW = sizeof(T) == 4 ? 3 : 6; };   // 128-bit words of a half-spinor
+
+__device__ __forceinline__ void half_to_words(const cx<float> (&h)[2][3], float4 (&w)[3]) {
+    w[0] = make_float4(h[0][0].re, h[0][0].im, h[0][1].re, h[0][1].im);
+    w[1] = make_float4(h[0][2].re, h[0][2].im, h[1][0].re, h[1][0].im);
+    w[2] = make_float4(h[1][1].re, h[1][1].im, h[1][2].re, h[1][2].im);
+}
+__device__ __forceinline__ void words_to_half(const float4 (&w)[3], cx<float> (&h)[2][3]) {
+    h[0][0] = {w[0].x, w[0].y}; h[0][1] = {w[0].z, w[0].w};
+    h[0][2] = {w[1].x, w[1].y}; h[1][0] = {w[1].z, w[1].w};
+    h[1][1] = {w[2].x, w[2].y}; h[1][2] = {w[2].z, w[2].w};
+}
+// slot (kind, site) of one exchange buffer: words [kind][w][site], consecutive lanes on consecutive 128-bit words
+template <typename T, int NT>
+__device__ __forceinline__ void put_half(typename Prec<T>::Vec* buf, int kind, int site, const cx<T> (&h)[2][3]) {
+    constexpr int NW = HalfWords<T>::NW;
+    typename Prec<T>::Vec w[NW];
+    half_to_words(h, w);
+#pragma unroll
+    for (int i = 0; i < NW; i++) buf[(kind * NW + i) * NT + site] = w[i];
+}
+template <typename T, int NT>
+__device__ __forceinline__ void get_half(const typename Prec<T>::Vec* buf, int kind, int site, cx<T> (&h)[2][3]) {
+    constexpr int NW = HalfWords<T>::NW;
+    typename Prec<T>::Vec w[NW];
+#pragma unroll
+    for (int i = 0; i < NW; i++) w[i] = buf[(kind * NW + i) * NT + site];
+    words_to_half(w, h);
+}
+
+__device__ __forceinline__ float shfl_real(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+template <typename T> __device__ __forceinline__ void shfl_half(cx<T> (&h)[2][3], int src) {
+#pragma unroll
+    for (int s = 0; s < 2; s++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            h[s][c].re = shfl_real(h[s][c].re, src);
+            h[s][c].im = shfl_real(h[s][c].im, src);
+        }
+}
+
+// a link kept in registers between its two uses (send phase: U^dagger on the own spinor; receive phase: U on the neighbour's).
+// fp32 keeps the whole matrix; fp64, short of registers, keeps two rows and rebuilds the third (eq. 2.3) at the second use.
+template <typename T> struct KeptLink {
+    static constexpr int ROWS = sizeof(T) == 4 ? 3 : 2;
+    cx<T> r[ROWS][3];
+    __device__ __forceinline__ void keep(const cx<T> (&U)[3][3]) {
+#pragma unroll
+        for (int i = 0; i < ROWS; i++)
+#pragma unroll
+            for (int j = 0; j < 3; j++) r[i][j] = U[i][j];
+    }
+    __device__ __forceinline__ void get(cx<T> (&U)[3][3]) const {
+#pragma unroll
+        for (int i = 0; i < ROWS; i++)
+#pragma unroll
+            for (int j = 0; j < 3; j++) U[i][j] = r[i][j];
+        if (ROWS == 2) third_row(U);
+    }
+};
+
+// cp.async (LDGSTS): 16 bytes global -> shared without passing through registers; .cg = cached in L2 only (streamed data)
+template <int BYTES> __device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");   // fp32 recon 18: 64-bit words
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// The halo slot of a tile-face thread: the spinor (and, for a backward face, the link) of its neighbour outside the tile,
+// fetched by cp.async one phase ahead: words [NV spinor planes][NT] then [NL link words][NT].
+template <typename T, int RECON, int MU, int NT>
+__device__ __forceinline__ void issue_halo(unsigned char* hal, const typename Prec<T>::Vec* __restrict__ in,
+                                           const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, long long V, int site,
+                                           bool face_bwd, bool face_fwd, long long s_bwd, long long s_fwd) {
+    using Vec = typename Prec<T>::Vec;
+    using LL = LinkLayout<T, RECON>;
+    Vec* hs = reinterpret_cast<Vec*>(hal);
+    typename LL::LVec* hl = reinterpret_cast<typename LL::LVec*>(hal + (size_t)Prec<T>::NV * NT * sizeof(Vec));
+    if (face_fwd || face_bwd) {
+        const long long sn = face_fwd ? s_fwd : s_bwd;
+#pragma unroll
+        for (int p = 0; p < Prec<T>::NV; p++) cp_async<16>(&hs[p * NT + site], in + p * V + sn);
+    }
+    if (face_bwd) {
+#pragma unroll
+        for (int p = 0; p < LL::NL; p++) cp_async<sizeof(typename LL::LVec)>(&hl[p * NT + site], gauge + ((long long)MU * LL::NL + p) * V + s_bwd);
+    }
+}
+
+// One direction mu in {1, 2} of the send phase of a site: the two half-spinors its in-tile neighbours need, and, on a tile
+// face, the half-spinor this site itself needs from outside the tile (neighbour data from the halo slot).
+//   slot kinds K = "h- of my forward neighbour" (read in the forward hop), K + 1 = "w of my backward neighbour"
+template <typename T, int RECON, int MU, int NT, int K>
+__device__ __forceinline__ void send_dir(typename Prec<T>::Vec* buf, const unsigned char* hal, const cx<T> (&phi)[12],
+                                         const cx<T> (&U)[3][3], int site, int slot_bwd, int slot_fwd, bool face_bwd, bool face_fwd) {
+    using Vec = typename Prec<T>::Vec;
+    using LL = LinkLayout<T, RECON>;
+    cx<T> h[2][3], g[2][3];
+    if (slot_bwd >= 0) {   // my h- goes to the site behind me: it is ITS forward neighbour's projection
+        project<T, MU, -1>(phi, T(1), h);
+        put_half<T, NT>(buf, K, slot_bwd, h);
+    }
+    if (slot_fwd >= 0) {   // my complete backward-hop product goes to the site in front of me
+        project<T, MU, +1>(phi, T(1), h);
+        mul_Udag(U, h, g);
+        put_half<T, NT>(buf, K + 1, slot_fwd, g);
+    }
+    if (face_fwd || face_bwd) {
+        const Vec* hs = reinterpret_cast<const Vec*>(hal);
+        Vec w[Prec<T>::NV];
+#pragma unroll
+        for (int p = 0; p < Prec<T>::NV; p++) w[p] = hs[p * NT + site];
+        cx<T> psi[12];
+        words_to_cx(w, psi);
+        if (face_fwd) {    // forward neighbour outside the tile
+            project<T, MU, -1>(psi, T(1), h);
+            put_half<T, NT>(buf, K, site, h);
+        } else {           // backward neighbour outside the tile: its spinor and its link
+            const typename LL::LVec* hl = reinterpret_cast<const typename LL::LVec*>(hal + (size_t)Prec<T>::NV * NT * sizeof(Vec));
+            typename LL::LVec lw[LL::NL];
+#pragma unroll
+            for (int p = 0; p < LL::NL; p++) lw[p] = hl[p * NT + site];
+            cx<T> Ub[3][3];
+            reconstruct_link<T, RECON>(lw, Ub);
+            project<T, MU, +1>(psi, T(1), h);
+            mul_Udag(Ub, h, g);
+            put_half<T, NT>(buf, K + 1, site, g);
+        }
+    }
+}
+
+template <typename T, int MU, int NT, int K>
+__device__ __forceinline__ void recv_dir(const typename Prec<T>::Vec* buf, const cx<T> (&U)[3][3], int site, cx<T> (&acc)[12]) {
+    cx<T> h[2][3], g[2][3];
+    get_half<T, NT>(buf, K, site, h);        // (1 - gamma_mu) phi(x + mu^)
+    mul_U(U, h, g);
+    accumulate<T, MU, -1>(g, acc);
+    get_half<T, NT>(buf, K + 1, site, g);    // U_mu(x - mu^)^dagger (1 + gamma_mu) phi(x - mu^)
+    accumulate<T, MU, +1>(g, acc);
+}
+
+// the thread's private link slot: words [mu][w][site].  take_link reads link mu of the current slice from the slot, rebuilds
+// the matrix, and (when `next` is a site of the next slice) refills the slot with the next slice's words by cp.async - the
+// in-flight link data of a whole time-slice lives in shared memory, not in registers.
+template <typename T, int RECON, int NT>
+__device__ __forceinline__ void take_link(typename LinkLayout<T, RECON>::LVec* lnk, const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge,
+                                          long long V, int mu, int site, bool refill, long long s_next, cx<T> (&U)[3][3]) {
+    using LL = LinkLayout<T, RECON>;
+    typename LL::LVec w[LL::NL];
+#pragma unroll
+    for (int p = 0; p < LL::NL; p++) w[p] = lnk[(mu * LL::NL + p) * NT + site];
+    reconstruct_link<T, RECON>(w, U);
+    if (refill) {
+        const typename LL::LVec* src = gauge + (long long)mu * LL::NL * V + s_next;
+#pragma unroll
+        for (int p = 0; p < LL::NL; p++) cp_async<sizeof(typename LL::LVec)>(&lnk[(mu * LL::NL + p) * NT + site], src + p * V);
+    }
+}
+
+// The vectors of the fused update out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3 at this thread's site, loaded BEFORE the last barrier
+// of the slice and combined after it (out may alias any v_i: every v_i(x) is read before out(x) is written, by the same thread).
+// (fp64 has no registers to spare for this: there the vectors are loaded at use, after the barrier.)
+template <typename T, bool EPI> struct EpiVectors {
+    static constexpr bool EARLY = EPI && sizeof(T) == 4;
+    typename Prec<T>::Vec w[EARLY ? 3 : 1][Prec<T>::NV];
+    const typename Prec<T>::Vec* vs[3];
+    __device__ __forceinline__ void load(long long V, long long s, T s1, const typename Prec<T>::Vec* v1, T s2,
+                                         const typename Prec<T>::Vec* v2, T s3, const typename Prec<T>::Vec* v3) {
+        vs[0] = v1; vs[1] = v2; vs[2] = v3;
+        if (EARLY) {
+#pragma unroll
+            for (int j = 0; j < 3; j++)
+                if (vs[j]) {
+#pragma unroll
+                    for (int p = 0; p < Prec<T>::NV; p++) w[j][p] = vs[j][p * V + s];
+                }
+        }
+    }
+    __device__ __forceinline__ void finish(typename Prec<T>::Vec* out, long long V, long long s, const cx<T> (&acc)[12], T s0, T s1,
+                                           T s2, T s3) {
+        using Vec = typename Prec<T>::Vec;
+        constexpr int NV = Prec<T>::NV;
+        cx<T> res[12];
+#pragma unroll
+        for (int i = 0; i < 12; i++) {
+            const T sg = (i < 6) ? T(-0.5) : T(0.5);   // gamma5 [ -1/2 acc ]
+            res[i].re = sg * acc[i].re;
+            res[i].im = sg * acc[i].im;
+        }
+        Vec o[NV];
+        cx_to_words(res, o);
+        if (EPI) {
+            T* wr = reinterpret_cast<T*>(o);
+#pragma unroll
+            for (int i = 0; i < 24; i++) wr[i] *= s0;
+            const T ss[3] = {s1, s2, s3};
+#pragma unroll
+            for (int j = 0; j < 3; j++)
+                if (vs[j]) {
+                    if (EARLY) {
+                        const T* ar = reinterpret_cast<const T*>(w[j]);
+#pragma unroll
+                        for (int i = 0; i < 24; i++) wr[i] = fma(ss[j], ar[i], wr[i]);
+                    } else {
+#pragma unroll
+                        for (int p = 0; p < NV; p++) {
+                            const Vec a = vs[j][p * V + s];
+                            const T* ar = reinterpret_cast<const T*>(&a);
+#pragma unroll
+                            for (int i = 0; i < 24 / NV; i++) wr[p * (24 / NV) + i] = fma(ss[j], ar[i], wr[p * (24 / NV) + i]);
+                        }
+                    }
+                }
+        }
+#pragma unroll
+        for (int p = 0; p < NV; p++) out[p * V + s] = o[p];
+    }
+};
+
+// Synchronisation of the exchange.  In a 2 x 2 x 32 tile a warp is one x3 row and has exactly ONE partner warp per direction
+// (the other row of the pair), so a 64-thread named barrier per pair replaces the CTA-wide barrier, with two meetings per
+// direction and slice: "the partner has finished its previous receive" before the send, "data is in place" after it.  The
+// first meeting orders EVERYTHING the partner did before it, so x1 and x2 can share one exchange buffer: a site's slots are
+// written by its x1 partner only after the site's own x2 receive of the last slice, and by its x2 partner only after its
+// own x1 receive of this slice.
+template <int B1, int B2, int L3> struct PairSync { static constexpr bool value = (B1 == 2 && B2 == 2 && L3 == 32); };
+__device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+
+template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB>
+__global__ void __launch_bounds__(B1* B2* L3, MINB)
+    wilson_Q_tile_kernel(typename Prec<T>::Vec* out, const typename Prec<T>::Vec* __restrict__ in,
+                         const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, TileGeom G, T mass_term, T s0, T s1,
+                         const typename Prec<T>::Vec* v1, T s2, const typename Prec<T>::Vec* v2, T s3,
+                         const typename Prec<T>::Vec* v3) {
+    using Vec = typename Prec<T>::Vec;
+    using LL = LinkLayout<T, RECON>;
+    using LVec = typename LL::LVec;
+    constexpr int NT = B1 * B2 * L3;
+    constexpr int NW = HalfWords<T>::NW;
+    // exchange kinds: x1 uses 0, 1; x2 uses 2, 3 - or 0, 1 again where the pair barriers make one buffer enough
+    constexpr int NK = PairSync<B1, B2, L3>::value ? 2 : 4;
+    constexpr int K2 = PairSync<B1, B2, L3>::value ? 0 : 2;
+    constexpr int ROW1 = B2 * L3;   // slot distance of x1 neighbours
+    constexpr int ROW2 = L3;        // slot distance of x2 neighbours
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Vec* xbuf = reinterpret_cast<Vec*>(smem_raw);                                  // exchange: [NK kinds][NW][NT]
+    LVec* lnk = reinterpret_cast<LVec*>(smem_raw + (size_t)NK * NW * NT * sizeof(Vec));   // links: [4 mu][NL][NT]
+    unsigned char* hal = smem_raw + (size_t)NK * NW * NT * sizeof(Vec) + (size_t)4 * LL::NL * NT * sizeof(LVec);   // halo slot
+
+    const int site = threadIdx.x;
+    const int x3 = site % L3, r2 = (site / L3) % B2, r1 = site / (L3 * B2);
+    const int tile = blockIdx.x % G.ntile, seg = blockIdx.x / G.ntile;
+    const int x1 = (tile / G.nt2) * B1 + r1, x2 = (tile % G.nt2) * B2 + r2;
+    const long long S1 = (long long)G.L2 * L3, S2 = L3;
+    const long long ss = ((long long)x1 * G.L2 + x2) * L3 + x3;
+    const int ts = seg * G.seg_base + (seg < G.seg_rem ? seg : G.seg_rem);
+    const int len = G.seg_base + (seg < G.seg_rem ? 1 : 0);
+
+    // the links of the segment's first slice start their way into the thread's slot
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++)
+#pragma unroll
+        for (int p = 0; p < LL::NL; p++)
+            cp_async<sizeof(LVec)>(&lnk[(mu * LL::NL + p) * NT + site], gauge + ((long long)mu * LL::NL + p) * G.V + ts * G.S0 + ss);
+
+    // neighbours in x1 / x2: inside the tile (slot index), or outside (global site offset within the slice)
+    const bool wrap1 = (G.L1 == B1), wrap2 = (G.L2 == B2);
+    const int slot_b1 = (r1 > 0) ? site - ROW1 : (wrap1 ? site + (B1 - 1) * ROW1 : -1);
+    const int slot_f1 = (r1 < B1 - 1) ? site + ROW1 : (wrap1 ? site - (B1 - 1) * ROW1 : -1);
+    const int slot_b2 = (r2 > 0) ? site - ROW2 : (wrap2 ? site + (B2 - 1) * ROW2 : -1);
+    const int slot_f2 = (r2 < B2 - 1) ? site + ROW2 : (wrap2 ? site - (B2 - 1) * ROW2 : -1);
+    const bool face_b1 = slot_b1 < 0, face_f1 = slot_f1 < 0, face_b2 = slot_b2 < 0, face_f2 = slot_f2 < 0;
+    const long long ss_b1 = (x1 == 0) ? ss + (long long)(G.L1 - 1) * S1 : ss - S1;
+    const long long ss_f1 = (x1 == G.L1 - 1) ? ss - (long long)(G.L1 - 1) * S1 : ss + S1;
+    const long long ss_b2 = (x2 == 0) ? ss + (long long)(G.L2 - 1) * S2 : ss - S2;
+    const long long ss_f2 = (x2 == G.L2 - 1) ? ss - (long long)(G.L2 - 1) * S2 : ss + S2;
+    // x3 neighbours: lanes of the same warp (a warp holds 32 / L3 complete x3 rows)
+    const int lane = threadIdx.x & 31;
+    const int lane_f3 = (lane & ~(L3 - 1)) | ((lane + 1) & (L3 - 1));
+    const int lane_b3 = (lane & ~(L3 - 1)) | ((lane + L3 - 1) & (L3 - 1));
+
+    issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, ts * G.S0 + ss_b1, ts * G.S0 + ss_f1);
+    cp_async_commit();
+
+    cx<T> phi_c[12], w0[2][3];
+    {
+        // the backward time hop of the segment's first slice: U_0(x, t-1)^dagger (1 + gamma_0) phi(x, t-1)
+        const int tp = (ts == 0) ? G.L0 - 1 : ts - 1;
+        cx<T> psi[12], U[3][3], h[2][3];
+        load_spinor<T>(in, G.V, tp * G.S0 + ss, psi);
+        load_link<T, RECON>(gauge, G.V, 0, tp * G.S0 + ss, U);
+        project<T, 0, +1>(psi, (ts == 0) ? T(G.bc) : T(1), h);
+        mul_Udag(U, h, w0);
+        load_spinor<T>(in, G.V, ts * G.S0 + ss, phi_c);
+    }
+
+    for (int i = 0; i < len; i++) {
+        const int t = ts + i;
+        const long long st = t * G.S0;
+        const long long s = st + ss;
+        const bool more = (i + 1 < len);           // the next slice belongs to this segment: prefetch its links
+        const long long s_next = s + G.S0;         // (only used when `more`: t + 1 < L0 then)
+        cx<T> phi_n[12];
+        load_spinor<T>(in, G.V, ((t == G.L0 - 1) ? 0 : st + G.S0) + ss, phi_n);   // next slice of this column
+        cp_async_wait_all();                        // this slice's link words and x1 halo (issued one slice ago) have landed
+
+        cx<T> acc[12];
+        {
+            const T f = T(-2) * mass_term;   // -1/2 acc = (4+m) phi - 1/2 sum(hops)
+#pragma unroll
+            for (int k = 0; k < 12; k++) acc[k] = {f * phi_c[k].re, f * phi_c[k].im};
+        }
+        KeptLink<T> kept;
+        // ---- x1: send
+        if (PairSync<B1, B2, L3>::value) pair_barrier(1 + r2);   // the partner row has finished last slice's x1 receive
+        {
+            cx<T> U[3][3];
+            take_link<T, RECON, NT>(lnk, gauge, G.V, 1, site, more, s_next, U);
+            kept.keep(U);
+            send_dir<T, RECON, 1, NT, 0>(xbuf, hal, phi_c, U, site, slot_b1, slot_f1, face_b1, face_f1);
+            issue_halo<T, RECON, 2, NT>(hal, in, gauge, G.V, site, face_b2, face_f2, st + ss_b2, st + ss_f2);   // the slot is free again
+            cp_async_commit();
+        }
+        // ---- x3: the neighbours are lanes of this warp
+        {
+            cx<T> U[3][3], h[2][3], g[2][3];
+            take_link<T, RECON, NT>(lnk, gauge, G.V, 3, site, more, s_next, U);
+            project<T, 3, -1>(phi_c, T(1), h);
+            shfl_half(h, lane_f3);             // (1 - gamma_3) phi(x + 3^)
+            mul_U(U, h, g);
+            accumulate<T, 3, -1>(g, acc);
+            project<T, 3, +1>(phi_c, T(1), h);
+            mul_Udag(U, h, g);
+            shfl_half(g, lane_b3);             // U_3(x - 3^)^dagger (1 + gamma_3) phi(x - 3^)
+            accumulate<T, 3, +1>(g, acc);
+        }
+        if (PairSync<B1, B2, L3>::value) pair_barrier(1 + r2);   // x1 half-spinors are in place
+        else __syncthreads();                  // ... (and everybody's x2 receive of the last slice is finished)
+        {
+            cx<T> U[3][3];
+            kept.get(U);
+            recv_dir<T, 1, NT, 0>(xbuf, U, site, acc);
+        }
+        // ---- x2: send
+        if (PairSync<B1, B2, L3>::value) pair_barrier(3 + r1);   // the partner row has finished last slice's x2 receive
+        {
+            cx<T> U[3][3];
+            take_link<T, RECON, NT>(lnk, gauge, G.V, 2, site, more, s_next, U);
+            kept.keep(U);
+            cp_async_wait_all();               // the x2 halo
+            send_dir<T, RECON, 2, NT, K2>(xbuf, hal, phi_c, U, site, slot_b2, slot_f2, face_b2, face_f2);
+            if (more) issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, st + G.S0 + ss_b1, st + G.S0 + ss_f1);
+        }
+        // ---- x0: this thread's own column
+        {
+            cx<T> U[3][3], h[2][3], g[2][3];
+            accumulate<T, 0, +1>(w0, acc);     // carried from the previous slice
+            take_link<T, RECON, NT>(lnk, gauge, G.V, 0, site, more, s_next, U);
+            project<T, 0, -1>(phi_n, (t == G.L0 - 1) ? T(G.bc) : T(1), h);
+            mul_U(U, h, g);
+            accumulate<T, 0, -1>(g, acc);
+            project<T, 0, +1>(phi_c, (t == G.L0 - 1) ? T(G.bc) : T(1), h);
+            mul_Udag(U, h, w0);                // the next slice's backward time hop
+        }
+        cp_async_commit();
+        EpiVectors<T, EPI> ev;
+        ev.load(G.V, s, s1, v1, s2, v2, s3, v3);   // the fused update's vectors are on their way while the barrier is met
+        if (PairSync<B1, B2, L3>::value) pair_barrier(3 + r1);   // x2 half-spinors are in place
+        else __syncthreads();                  // ... (and everybody's x1 receive of this slice is finished)
+        {
+            cx<T> U[3][3];
+            kept.get(U);
+            recv_dir<T, 2, NT, K2>(xbuf, U, site, acc);
+        }
+        ev.finish(out, G.V, s, acc, s0, s1, s2, s3);
+#pragma unroll
+        for (int k = 0; k < 12; k++) phi_c[k] = phi_n[k];
+    }
+}
+
+// the number of segments along x0 that fills the machine best: CTAs = ntile * nseg are handed to `slots` resident CTA
+// slots in rounds; a short segment pays its prologue (one extra spinor + link read per column) more often
+int choose_segments(int L0, int ntile, int slots) {
+    int best = 1;
+    double best_eff = 0.0;
+    for (int nseg = 1; nseg <= L0; nseg++) {
+        const long long ctas = (long long)ntile * nseg;
+        const long long rounds = (ctas + slots - 1) / slots;
+        const int longest = (L0 + nseg - 1) / nseg;
+        // time ~ rounds * (longest + prologue), work = L0 * ntile / slots
+        const double eff = ((double)L0 * ntile / slots) / ((double)rounds * (longest + 0.6));
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = nseg; }
+    }
+    return best;
+}
+
+template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB>
+int launch_tile(nd_ctx* ctx, void* out, const void* in, double m, double s0, double s1, const void* v1, double s2, const void* v2,
+                double s3, const void* v3) {
+    using Vec = typename Prec<T>::Vec;
+    using LVec = typename LinkLayout<T, RECON>::LVec;
+    constexpr int NT = B1 * B2 * L3;
+    constexpr int NW = HalfWords<T>::NW;
+    // exchange buffer(s) + 4 link slots + halo slot (spinor + 1 link)
+    constexpr size_t smem = (size_t)(PairSync<B1, B2, L3>::value ? 2 : 4) * NW * NT * sizeof(Vec) +
+                            (size_t)5 * LinkLayout<T, RECON>::NL * NT * sizeof(LVec) + (size_t)Prec<T>::NV * NT * sizeof(Vec);
+    TileGeom G;
+    G.L0 = ctx->dims[0]; G.L1 = ctx->dims[1]; G.L2 = ctx->dims[2];
+    G.V = ctx->V;
+    G.S0 = (long long)ctx->dims[1] * ctx->dims[2] * ctx->dims[3];
+    G.bc = ctx->bc;
+    G.nt2 = G.L2 / B2;
+    G.ntile = (G.L1 / B1) * G.nt2;
+    auto kern = wilson_Q_tile_kernel<T, RECON, EPI, B1, B2, L3, MINB>;
+    int& per_sm = ctx->tile_ctas_per_sm[EPI ? 1 : 0];
+    if (per_sm == 0) {
+        ND_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int n = 0;
+        ND_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, NT, smem));
+        if (n < 1) return nd_fail(ctx, ND_ERR_CUDA, "tiled stencil does not fit on an SM");
+        per_sm = n;
+    }
+    const int nseg = choose_segments(G.L0, G.ntile, per_sm * ctx->num_sms);
+    G.seg_base = G.L0 / nseg;
+    G.seg_rem = G.L0 % nseg;
+    const unsigned blocks = (unsigned)(G.ntile * nseg);
+    kern<<<blocks, NT, smem, ctx->stream>>>((Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(s0), T(s1),
+                                            (const Vec*)v1, T(s2), (const Vec*)v2, T(s3), (const Vec*)v3);
+    ND_LAUNCHED(ctx);
+    return ND_OK;
+}
+
+// fp32 only (see ndi_tile_supported).  Registers per thread: the plain kernel fits 3 CTAs of 128 threads per SM (168
+// registers), the fused-epilogue kernel holds the three update vectors of its site as well and runs 2 CTAs per SM.
+template <int RECON>
+int launch_tile_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
+                      const void* v2, double s3, const void* v3) {
+    if (ctx->dims[3] == 32) {
+        if (epi) return launch_tile<float, RECON, true, 2, 2, 32, 2>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile<float, RECON, false, 2, 2, 32, 3>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+    }
+    if (epi) return launch_tile<float, RECON, true, 2, 4, 16, 2>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile<float, RECON, false, 2, 4, 16, 3>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+}
+
+}  // namespace
+
+// Lattices the tiled kernel takes: fp32 (in fp64 a site's state - accumulators, the current and the next spinor of the column,
+// the carried time hop, a kept link - does not fit the register file at a useful occupancy: measured 357 / 600 us per launch
+// on 32^3x64 against 349 / 498 us of the site-per-thread kernel), x3 extent 32 (tile 2 x 2 x 32) or
+// 16 (tile 2 x 4 x 16), even x1 / x2 extents divisible by the tile, and enough tiles to give every SM work.
+bool ndi_tile_supported(const nd_ctx* ctx) {
+    const int L1 = ctx->dims[1], L2 = ctx->dims[2], L3 = ctx->dims[3];
+    if (ctx->prec != 32) return false;
+    int b1 = 2, b2;
+    if (L3 == 32) b2 = 2;
+    else if (L3 == 16) b2 = 4;
+    else return false;
+    if (L1 % b1 != 0 || L2 % b2 != 0) return false;
+    return (long long)(L1 / b1) * (L2 / b2) * ctx->dims[0] >= 8LL * ctx->num_sms;
+}
+
+int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
+                     const void* v2, double s3, const void* v3) {
+    if (ctx->recon == 18) return launch_tile_shape<18>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);   // (fused epilogue only)
+    if (ctx->recon == 12) return launch_tile_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+}

@@ -140,3 +140,25 @@ def test_projector_error_matches_oracle():
     kappa, bound, _ = nd.projector_error([1.0], [0.1], [2.0])
     assert abs(kappa[0] - 0.1) < 1e-16 and abs(bound[0] - 0.12 / 0.76) < 1e-15 and kappa[1] == 0 and bound[1] == 0
     assert np.isinf(nd.projector_error([1.0], [0.5], [2.0])[1][0])
+
+
+def test_choose_l_matches_oracle():
+    """nd_choose_l (library, R17) vs the oracle's independent gap rule on hand-made and random spectra."""
+    import paper_1010_5636_b200 as nd
+    from oracle import lowmodes as olow
+
+    a = np.array([0.10, 0.11, 0.30, 0.301, 0.302, 0.50, 0.90])
+    for lo, hi in ((3, 5), (2, 4), (3, 4), (4, 4), (1, 6)):
+        l, gap = nd.choose_l(a, lo, hi)
+        lo_, gap_ = olow.choose_l(a, lo, hi)
+        assert l == lo_ and abs(gap - gap_) < 1e-15
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        k = int(rng.integers(3, 80))
+        a = np.sort(rng.random(k))
+        lo = int(rng.integers(1, k - 1))
+        hi = int(rng.integers(lo, k - 1))
+        assert nd.choose_l(a, lo, hi)[0] == olow.choose_l(a, lo, hi)[0]
+    for bad in ((a[::-1], 1, 2), (a, 0, 2), (a, 3, 2), (a, 1, len(a))):
+        with pytest.raises(nd.NDError):
+            nd.choose_l(*bad)

@@ -118,9 +118,9 @@ def test_gap_rule_lowers_kappa_for_a_perturbed_low_space(dense_4x4_smooth):
     V = olow.orthonormalise([W[:, i].reshape(shape) + 2e-7 * (rng.standard_normal(shape) + 1j * rng.standard_normal(shape))
                              for i in order[:k]])
     nu, U = sign.rayleigh_ritz_Q(Q, V)
-    o = np.argsort(np.abs(nu))
-    nu, U = nu[o], [U[i] for i in o]
     rho = sign.residues(Q, nu, U)
+    o = np.argsort(np.hypot(nu, rho))            # the block is ordered by a_j = ||Q u_j|| (R17)
+    nu, U, rho = nu[o], [U[i] for i in o], rho[o]
     ec = olow.error_control(nu, rho, lo, hi)
     assert ec["l"] == l_gap                                              # Ritz values this accurate reproduce the exact choice
     bad = olow.error_control(nu, rho, l_bad, l_bad)
