@@ -70,6 +70,15 @@ ND_API int nd_set_stream(nd_ctx* ctx, void* stream);
 ND_API long long nd_volume(const nd_ctx* ctx);          /* number of sites V */
 ND_API size_t nd_spinor_bytes(const nd_ctx* ctx);       /* bytes of one device SoA spinor = 24 * V * prec/8 */
 ND_API size_t nd_gauge_bytes(const nd_ctx* ctx);        /* bytes of the compressed device gauge field */
+/* Which kernel applies the stencil (csrc/wilson.cu, csrc/wilson_tile.cu).  ND_STENCIL_AUTO (default)
+ * picks the fastest one measured for the context: the tiled marching kernel (neighbour exchange through shared memory,
+ * cp.async prefetch) for fp32 lattices it supports - x3 extent 32, even x1 / x2 extents, at least 8 tiles per SM - and the
+ * site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The other values force one kernel, for parity tests and
+ * for timing the variants against each other; ND_ERR_BAD_ARG if the context cannot run it.  Cached CUDA graphs are dropped.
+ * nd_get_stencil_variant returns the variant in effect (never ND_STENCIL_AUTO). */
+enum { ND_STENCIL_AUTO = 0, ND_STENCIL_SITE = 1, ND_STENCIL_TILE = 2, ND_STENCIL_TILE_TMA = 3 };
+ND_API int nd_set_stencil_variant(nd_ctx* ctx, int variant);
+ND_API int nd_get_stencil_variant(const nd_ctx* ctx);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 ND_API long long nd_launch_count(const nd_ctx* ctx);
 

@@ -35,6 +35,8 @@ SIGNATURES = {
     "nd_spinor_bytes": (_c_sz, [_c_vp]),
     "nd_gauge_bytes": (_c_sz, [_c_vp]),
     "nd_launch_count": (_c_ll, [_c_vp]),
+    "nd_set_stencil_variant": (_c_int, [_c_vp, _c_int]),
+    "nd_get_stencil_variant": (_c_int, [_c_vp]),
     "nd_set_gauge": (_c_int, [_c_vp, _c_vp, _c_int, _c_int]),
     "nd_get_gauge": (_c_int, [_c_vp, _c_vp, _c_int]),
     "nd_gauge_stats": (_c_int, [_c_vp, _pd]),
@@ -224,6 +226,15 @@ class Context:
         shape = (24 * self.V,) if count is None else (int(count), 24 * self.V)
         with torch.cuda.stream(self.stream):
             return torch.empty(shape, dtype=self.real_dtype, device=self.torch_device)
+
+    STENCIL = {"auto": 0, "site": 1, "tile": 2, "tile_tma": 3}
+
+    def set_stencil_variant(self, name):
+        self._chk(self.lib.nd_set_stencil_variant(self._h, self.STENCIL[name]))
+
+    def get_stencil_variant(self):
+        v = int(self.lib.nd_get_stencil_variant(self._h))
+        return {n: k for k, n in self.STENCIL.items()}[v]
 
     def launch_count(self):
         return int(self.lib.nd_launch_count(self._h))

@@ -75,8 +75,9 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->num_sms = 148;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     ctx->err[0] = 0;
-    ctx->tile_ctas_per_sm[0] = ctx->tile_ctas_per_sm[1] = 0;
-    ctx->use_tile_kernel = ndi_tile_supported(ctx);
+    for (int i = 0; i < 4; i++) ctx->tile_ctas_per_sm[i] = 0;
+    ctx->tile_ok = ndi_tile_supported(ctx);
+    ctx->stencil_variant = ND_STENCIL_AUTO;
     // fp32 recon 18 is stored as 9 float2, everything else in 128-bit words: bytes = 4 * recon * V * prec/8
     ctx->gauge_bytes = (size_t)4 * recon * ctx->V * (prec / 8);
     cudaError_t e = cudaMalloc(&ctx->gauge, ctx->gauge_bytes);
@@ -121,6 +122,22 @@ extern "C" int nd_set_stream(nd_ctx* ctx, void* stream) {
     ctx->stream = (cudaStream_t)stream;
     ndi_drop_graphs(ctx);
     return ND_OK;
+}
+
+extern "C" int nd_set_stencil_variant(nd_ctx* ctx, int variant) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (variant != ND_STENCIL_AUTO && variant != ND_STENCIL_SITE && variant != ND_STENCIL_TILE && variant != ND_STENCIL_TILE_TMA)
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: unknown variant %d", variant);
+    if ((variant == ND_STENCIL_TILE || variant == ND_STENCIL_TILE_TMA) && !ctx->tile_ok)
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: the tiled kernel needs fp32, x3 extent 32, even x1 / x2 extents and >= 8 tiles per SM");
+    ctx->stencil_variant = variant;
+    ndi_drop_graphs(ctx);
+    return ND_OK;
+}
+extern "C" int nd_get_stencil_variant(const nd_ctx* ctx) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (ctx->stencil_variant != ND_STENCIL_AUTO) return ctx->stencil_variant;
+    return ctx->tile_ok ? ND_STENCIL_TILE : ND_STENCIL_SITE;
 }
 
 extern "C" long long nd_volume(const nd_ctx* ctx) { return ctx ? ctx->V : 0; }

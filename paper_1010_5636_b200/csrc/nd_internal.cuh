@@ -59,8 +59,9 @@ struct nd_ctx {
     int hop_max_sites;  // lattices below this volume use the hop-parallel stencil (wilson.cu)
     int tile_lb[3];     // stencil CTA tile: log2 extents along x1, x2, x3
     int tile_threads;   // sites per tile (0: linear mapping)
-    bool use_tile_kernel;       // the tiled marching stencil (wilson_tile.cu) takes this lattice
-    int tile_ctas_per_sm[2];    // its resident CTAs per SM (plain / fused epilogue), 0 = not queried yet
+    bool tile_ok;               // the tiled marching stencil (wilson_tile.cu) takes this lattice
+    int stencil_variant;        // ND_STENCIL_* (nd_set_stencil_variant)
+    int tile_ctas_per_sm[4];    // resident CTAs per SM of the tiled kernel ({cp.async, TMA} x {plain, fused}), 0 = not queried yet
     char err[512];
 };
 

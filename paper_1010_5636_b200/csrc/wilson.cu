@@ -276,7 +276,9 @@ int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, doub
     }
     // the tiled marching kernel (wilson_tile.cu) where it is the faster one: fp32 on lattices it supports; with the
     // uncompressed recon-18 links (64-bit words in fp32) only the fused-epilogue variant wins (224 vs 199 us plain, 252 vs 276 us fused)
-    if (ctx->use_tile_kernel && (ctx->recon != 18 || epi)) return ndi_apply_Q_tile(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->recon != 18 || epi))
+                                                                : (ctx->stencil_variant != ND_STENCIL_SITE);
+    if (tile) return ndi_apply_Q_tile(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
 #define ND_DISPATCH(T, R) return launch_Q<T, R>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3)
     if (ctx->prec == 32) {
         if (ctx->recon == 18) ND_DISPATCH(float, 18);

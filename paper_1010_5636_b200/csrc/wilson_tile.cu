@@ -102,6 +102,35 @@ template <int BYTES> __device__ __forceinline__ void cp_async(void* smem_dst, co
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
+// TMA bulk copies (cp.async.bulk, SASS UBLKCP): a warp owns one x3 row of 32 sites, and every plane of that row is 32
+// consecutive 128-bit words both in global memory and in the row's shared-memory slot, so one lane moves a whole row-plane
+// (512 bytes) with one instruction; completion is counted in bytes on an mbarrier of the warp.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
+                 "r"(bytes), "r"(smem_u32(b))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(b)),
+        "r"(parity)
+        : "memory");
+}
+
 // The halo slot of a tile-face thread: the spinor (and, for a backward face, the link) of its neighbour outside the tile,
 // fetched by cp.async one phase ahead: words [NV spinor planes][NT] then [NL link words][NT].
 template <typename T, int RECON, int MU, int NT>
@@ -121,6 +150,33 @@ __device__ __forceinline__ void issue_halo(unsigned char* hal, const typename Pr
 #pragma unroll
         for (int p = 0; p < LL::NL; p++) cp_async<sizeof(typename LL::LVec)>(&hl[p * NT + site], gauge + ((long long)MU * LL::NL + p) * V + s_bwd);
     }
+}
+
+// the same with bulk copies: lanes 0..NV-1 move one spinor plane of the neighbour row each, lanes NV..NV+NL-1 one link word
+// (rows are warp-uniform: L3 = 32).  Returns the bytes issued (for the mbarrier's expect_tx, armed by the caller).
+template <typename T, int RECON, int MU, int NT>
+__device__ __forceinline__ void issue_halo_bulk(unsigned char* hal, const typename Prec<T>::Vec* __restrict__ in,
+                                                const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, long long V, int row0,
+                                                int lane, bool face_bwd, bool face_fwd, long long row_bwd, long long row_fwd,
+                                                unsigned long long* bar) {
+    using Vec = typename Prec<T>::Vec;
+    using LL = LinkLayout<T, RECON>;
+    Vec* hs = reinterpret_cast<Vec*>(hal);
+    typename LL::LVec* hl = reinterpret_cast<typename LL::LVec*>(hal + (size_t)Prec<T>::NV * NT * sizeof(Vec));
+    if (face_fwd || face_bwd) {
+        const long long sn = face_fwd ? row_fwd : row_bwd;
+        if (lane < Prec<T>::NV) bulk_g2s(&hs[lane * NT + row0], in + lane * V + sn, 32 * sizeof(Vec), bar);
+        else if (face_bwd && lane < Prec<T>::NV + LL::NL)
+            bulk_g2s(&hl[(lane - Prec<T>::NV) * NT + row0], gauge + ((long long)MU * LL::NL + (lane - Prec<T>::NV)) * V + row_bwd,
+                     32 * sizeof(typename LL::LVec), bar);
+    }
+}
+template <typename T, int RECON> __device__ __forceinline__ unsigned halo_bytes(bool face_bwd, bool face_fwd) {
+    using LL = LinkLayout<T, RECON>;
+    unsigned b = 0;
+    if (face_fwd || face_bwd) b += Prec<T>::NV * 32 * sizeof(typename Prec<T>::Vec);
+    if (face_bwd && !face_fwd) b += LL::NL * 32 * sizeof(typename LL::LVec);
+    return b;
 }
 
 // One direction mu in {1, 2} of the send phase of a site: the two half-spinors its in-tile neighbours need, and, on a tile
@@ -193,6 +249,22 @@ __device__ __forceinline__ void take_link(typename LinkLayout<T, RECON>::LVec* l
     }
 }
 
+// bulk variant: lanes 0..NL-1 refill one row-plane of the slot each (the whole warp has read its words before: __syncwarp)
+template <typename T, int RECON, int NT>
+__device__ __forceinline__ void take_link_bulk(typename LinkLayout<T, RECON>::LVec* lnk, const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge,
+                                               long long V, int mu, int site, int lane, bool refill, long long row_next,
+                                               unsigned long long* bar, cx<T> (&U)[3][3]) {
+    using LL = LinkLayout<T, RECON>;
+    typename LL::LVec w[LL::NL];
+#pragma unroll
+    for (int p = 0; p < LL::NL; p++) w[p] = lnk[(mu * LL::NL + p) * NT + site];
+    reconstruct_link<T, RECON>(w, U);
+    __syncwarp();
+    if (refill && lane < LL::NL)
+        bulk_g2s(&lnk[(mu * LL::NL + lane) * NT + (site - lane)], gauge + ((long long)mu * LL::NL + lane) * V + row_next,
+                 32 * sizeof(typename LL::LVec), bar);
+}
+
 // The vectors of the fused update out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3 at this thread's site, loaded BEFORE the last barrier
 // of the slice and combined after it (out may alias any v_i: every v_i(x) is read before out(x) is written, by the same thread).
 // (fp64 has no registers to spare for this: there the vectors are loaded at use, after the barrier.)
@@ -262,7 +334,7 @@ template <typename T, bool EPI> struct EpiVectors {
 template <int B1, int B2, int L3> struct PairSync { static constexpr bool value = (B1 == 2 && B2 == 2 && L3 == 32); };
 __device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 
-template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB>
+template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB, bool BULK>
 __global__ void __launch_bounds__(B1* B2* L3, MINB)
     wilson_Q_tile_kernel(typename Prec<T>::Vec* out, const typename Prec<T>::Vec* __restrict__ in,
                          const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, TileGeom G, T mass_term, T s0, T s1,
@@ -292,12 +364,29 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
     const int ts = seg * G.seg_base + (seg < G.seg_rem ? seg : G.seg_rem);
     const int len = G.seg_base + (seg < G.seg_rem ? 1 : 0);
 
+    // bulk mode: two mbarriers per warp - TOP: the next slice's four links and x1 halo; MID: this slice's x2 halo
+    __shared__ unsigned long long mbar[2][NT / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned long long* bar_top = &mbar[0][warp];
+    unsigned long long* bar_mid = &mbar[1][warp];
+    const int row0 = site - lane;                  // the row's first slot (BULK: L3 == 32, lane == x3)
+    const long long rr = ss - lane;                // ... and first site within a slice
+    if (BULK) {
+        if (lane == 0) { mbar_init(bar_top, 1); mbar_init(bar_mid, 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        __syncthreads();
+    }
     // the links of the segment's first slice start their way into the thread's slot
+    if (BULK) {
+        for (int j = lane; j < 4 * LL::NL; j += 32)   // (recon 18 has 36 row-planes)
+            bulk_g2s(&lnk[j * NT + row0], gauge + (long long)j * G.V + ts * G.S0 + rr, 32 * sizeof(LVec), bar_top);
+    } else {
 #pragma unroll
-    for (int mu = 0; mu < 4; mu++)
+        for (int mu = 0; mu < 4; mu++)
 #pragma unroll
-        for (int p = 0; p < LL::NL; p++)
-            cp_async<sizeof(LVec)>(&lnk[(mu * LL::NL + p) * NT + site], gauge + ((long long)mu * LL::NL + p) * G.V + ts * G.S0 + ss);
+            for (int p = 0; p < LL::NL; p++)
+                cp_async<sizeof(LVec)>(&lnk[(mu * LL::NL + p) * NT + site], gauge + ((long long)mu * LL::NL + p) * G.V + ts * G.S0 + ss);
+    }
 
     // neighbours in x1 / x2: inside the tile (slot index), or outside (global site offset within the slice)
     const bool wrap1 = (G.L1 == B1), wrap2 = (G.L2 == B2);
@@ -311,12 +400,17 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
     const long long ss_b2 = (x2 == 0) ? ss + (long long)(G.L2 - 1) * S2 : ss - S2;
     const long long ss_f2 = (x2 == G.L2 - 1) ? ss - (long long)(G.L2 - 1) * S2 : ss + S2;
     // x3 neighbours: lanes of the same warp (a warp holds 32 / L3 complete x3 rows)
-    const int lane = threadIdx.x & 31;
     const int lane_f3 = (lane & ~(L3 - 1)) | ((lane + 1) & (L3 - 1));
     const int lane_b3 = (lane & ~(L3 - 1)) | ((lane + L3 - 1) & (L3 - 1));
 
-    issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, ts * G.S0 + ss_b1, ts * G.S0 + ss_f1);
-    cp_async_commit();
+    const unsigned top_bytes = 4 * LL::NL * 32 * sizeof(LVec) + halo_bytes<T, RECON>(face_b1, face_f1);
+    if (BULK) {
+        issue_halo_bulk<T, RECON, 1, NT>(hal, in, gauge, G.V, row0, lane, face_b1, face_f1, ts * G.S0 + ss_b1 - lane, ts * G.S0 + ss_f1 - lane, bar_top);
+        if (lane == 0) mbar_expect_tx(bar_top, top_bytes);
+    } else {
+        issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, ts * G.S0 + ss_b1, ts * G.S0 + ss_f1);
+        cp_async_commit();
+    }
 
     cx<T> phi_c[12], w0[2][3];
     {
@@ -338,7 +432,13 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
         const long long s_next = s + G.S0;         // (only used when `more`: t + 1 < L0 then)
         cx<T> phi_n[12];
         load_spinor<T>(in, G.V, ((t == G.L0 - 1) ? 0 : st + G.S0) + ss, phi_n);   // next slice of this column
-        cp_async_wait_all();                        // this slice's link words and x1 halo (issued one slice ago) have landed
+        // this slice's link words and x1 halo (issued one slice ago) have landed
+        if (BULK) {
+            mbar_wait(bar_top, i & 1);
+            if (more && lane == 0) mbar_expect_tx(bar_top, top_bytes);   // armed for the refills issued during this slice
+        } else {
+            cp_async_wait_all();
+        }
 
         cx<T> acc[12];
         {
@@ -351,16 +451,25 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
         if (PairSync<B1, B2, L3>::value) pair_barrier(1 + r2);   // the partner row has finished last slice's x1 receive
         {
             cx<T> U[3][3];
-            take_link<T, RECON, NT>(lnk, gauge, G.V, 1, site, more, s_next, U);
+            if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 1, site, lane, more, s_next - lane, bar_top, U);
+            else take_link<T, RECON, NT>(lnk, gauge, G.V, 1, site, more, s_next, U);
             kept.keep(U);
             send_dir<T, RECON, 1, NT, 0>(xbuf, hal, phi_c, U, site, slot_b1, slot_f1, face_b1, face_f1);
-            issue_halo<T, RECON, 2, NT>(hal, in, gauge, G.V, site, face_b2, face_f2, st + ss_b2, st + ss_f2);   // the slot is free again
-            cp_async_commit();
+            // the halo slot is free again: this slice's x2 halo
+            if (BULK) {
+                __syncwarp();
+                issue_halo_bulk<T, RECON, 2, NT>(hal, in, gauge, G.V, row0, lane, face_b2, face_f2, st + ss_b2 - lane, st + ss_f2 - lane, bar_mid);
+                if (lane == 0) mbar_expect_tx(bar_mid, halo_bytes<T, RECON>(face_b2, face_f2));
+            } else {
+                issue_halo<T, RECON, 2, NT>(hal, in, gauge, G.V, site, face_b2, face_f2, st + ss_b2, st + ss_f2);
+                cp_async_commit();
+            }
         }
         // ---- x3: the neighbours are lanes of this warp
         {
             cx<T> U[3][3], h[2][3], g[2][3];
-            take_link<T, RECON, NT>(lnk, gauge, G.V, 3, site, more, s_next, U);
+            if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 3, site, lane, more, s_next - lane, bar_top, U);
+            else take_link<T, RECON, NT>(lnk, gauge, G.V, 3, site, more, s_next, U);
             project<T, 3, -1>(phi_c, T(1), h);
             shfl_half(h, lane_f3);             // (1 - gamma_3) phi(x + 3^)
             mul_U(U, h, g);
@@ -381,24 +490,36 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
         if (PairSync<B1, B2, L3>::value) pair_barrier(3 + r1);   // the partner row has finished last slice's x2 receive
         {
             cx<T> U[3][3];
-            take_link<T, RECON, NT>(lnk, gauge, G.V, 2, site, more, s_next, U);
+            if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 2, site, lane, more, s_next - lane, bar_top, U);
+            else take_link<T, RECON, NT>(lnk, gauge, G.V, 2, site, more, s_next, U);
             kept.keep(U);
-            cp_async_wait_all();               // the x2 halo
+            // the x2 halo
+            if (BULK) mbar_wait(bar_mid, i & 1);
+            else cp_async_wait_all();
             send_dir<T, RECON, 2, NT, K2>(xbuf, hal, phi_c, U, site, slot_b2, slot_f2, face_b2, face_f2);
-            if (more) issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, st + G.S0 + ss_b1, st + G.S0 + ss_f1);
+            if (more) {
+                if (BULK) {
+                    __syncwarp();
+                    issue_halo_bulk<T, RECON, 1, NT>(hal, in, gauge, G.V, row0, lane, face_b1, face_f1, st + G.S0 + ss_b1 - lane,
+                                                     st + G.S0 + ss_f1 - lane, bar_top);
+                } else {
+                    issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, st + G.S0 + ss_b1, st + G.S0 + ss_f1);
+                }
+            }
         }
         // ---- x0: this thread's own column
         {
             cx<T> U[3][3], h[2][3], g[2][3];
             accumulate<T, 0, +1>(w0, acc);     // carried from the previous slice
-            take_link<T, RECON, NT>(lnk, gauge, G.V, 0, site, more, s_next, U);
+            if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 0, site, lane, more, s_next - lane, bar_top, U);
+            else take_link<T, RECON, NT>(lnk, gauge, G.V, 0, site, more, s_next, U);
             project<T, 0, -1>(phi_n, (t == G.L0 - 1) ? T(G.bc) : T(1), h);
             mul_U(U, h, g);
             accumulate<T, 0, -1>(g, acc);
             project<T, 0, +1>(phi_c, (t == G.L0 - 1) ? T(G.bc) : T(1), h);
             mul_Udag(U, h, w0);                // the next slice's backward time hop
         }
-        cp_async_commit();
+        if (!BULK) cp_async_commit();
         EpiVectors<T, EPI> ev;
         ev.load(G.V, s, s1, v1, s2, v2, s3, v3);   // the fused update's vectors are on their way while the barrier is met
         if (PairSync<B1, B2, L3>::value) pair_barrier(3 + r1);   // x2 half-spinors are in place
@@ -430,7 +551,7 @@ int choose_segments(int L0, int ntile, int slots) {
     return best;
 }
 
-template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB>
+template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB, bool BULK>
 int launch_tile(nd_ctx* ctx, void* out, const void* in, double m, double s0, double s1, const void* v1, double s2, const void* v2,
                 double s3, const void* v3) {
     using Vec = typename Prec<T>::Vec;
@@ -447,8 +568,8 @@ int launch_tile(nd_ctx* ctx, void* out, const void* in, double m, double s0, dou
     G.bc = ctx->bc;
     G.nt2 = G.L2 / B2;
     G.ntile = (G.L1 / B1) * G.nt2;
-    auto kern = wilson_Q_tile_kernel<T, RECON, EPI, B1, B2, L3, MINB>;
-    int& per_sm = ctx->tile_ctas_per_sm[EPI ? 1 : 0];
+    auto kern = wilson_Q_tile_kernel<T, RECON, EPI, B1, B2, L3, MINB, BULK>;
+    int& per_sm = ctx->tile_ctas_per_sm[(BULK ? 2 : 0) + (EPI ? 1 : 0)];
     if (per_sm == 0) {
         ND_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int n = 0;
@@ -471,12 +592,15 @@ int launch_tile(nd_ctx* ctx, void* out, const void* in, double m, double s0, dou
 template <int RECON>
 int launch_tile_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                       const void* v2, double s3, const void* v3) {
-    if (ctx->dims[3] == 32) {
-        if (epi) return launch_tile<float, RECON, true, 2, 2, 32, 2>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
-        return launch_tile<float, RECON, false, 2, 2, 32, 3>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+    // the prefetch of links and halos: cp.async (LDGSTS, one 16-byte copy per thread and word; the default: 144 / 223 us per
+    // launch on 32^3x64, recon 12) or TMA bulk copies (UBLKCP, one 512-byte row-plane per lane: 21 small requests per warp and
+    // slice keep the SM's TMA unit busier than the data path: 187 / 257 us) - ND_STENCIL_TILE_TMA selects the latter
+    if (ctx->stencil_variant == ND_STENCIL_TILE_TMA) {
+        if (epi) return launch_tile<float, RECON, true, 2, 2, 32, 2, true>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile<float, RECON, false, 2, 2, 32, 3, true>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
     }
-    if (epi) return launch_tile<float, RECON, true, 2, 4, 16, 2>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
-    return launch_tile<float, RECON, false, 2, 4, 16, 3>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+    if (epi) return launch_tile<float, RECON, true, 2, 2, 32, 2, false>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile<float, RECON, false, 2, 2, 32, 3, false>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
 }
 
 }  // namespace
@@ -488,10 +612,8 @@ int launch_tile_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi
 bool ndi_tile_supported(const nd_ctx* ctx) {
     const int L1 = ctx->dims[1], L2 = ctx->dims[2], L3 = ctx->dims[3];
     if (ctx->prec != 32) return false;
-    int b1 = 2, b2;
-    if (L3 == 32) b2 = 2;
-    else if (L3 == 16) b2 = 4;
-    else return false;
+    const int b1 = 2, b2 = 2;
+    if (L3 != 32) return false;
     if (L1 % b1 != 0 || L2 % b2 != 0) return false;
     return (long long)(L1 / b1) * (L2 / b2) * ctx->dims[0] >= 8LL * ctx->num_sms;
 }

@@ -1,0 +1,58 @@
+"""The tiled marching stencil (csrc/wilson_tile.cu: neighbour exchange through shared memory, cp.async / TMA-bulk prefetch)
+against the CPU oracle of eq. 2.1 and against the site-per-thread kernel, on lattices that exercise its index logic: several
+time segments per tile, the antiperiodic seam inside a segment, tiles on the lattice boundary in x1 / x2, and an x1 extent
+equal to the tile (both x1 neighbours are the same partner row)."""
+import numpy as np
+import pytest
+
+from lattice_inputs import gaussian_spinor
+from oracle import wilson_c
+from tests.gpu_common import TOL, make_context, rel_l2, round_to
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("dims,bc", [((40, 8, 16, 32), -1), ((152, 2, 16, 32), -1), ((38, 16, 8, 32), +1)])
+@pytest.mark.parametrize("recon", [12, 8, 18])
+def test_every_variant_matches_the_oracle(dims, bc, recon):
+    ctx, U = make_context(dims, 32, recon, bc, "smooth", eps=0.3)
+    assert ctx.get_stencil_variant() == "tile"                       # these lattices take the tiled kernel by default
+    psi = round_to(gaussian_spinor(dims), 32)
+    vecs = [round_to(gaussian_spinor(dims, seed=20 + i), 32) for i in range(3)]
+    x, y = ctx.pack_spinor(psi), ctx.new_spinor()
+    d = [ctx.pack_spinor(v) for v in vecs]
+    ref = wilson_c.apply_Q(psi, U, -1.6, bc)
+    s0, s1, s2, s3 = 0.37, -1.2, -1.0, 0.81
+    ref_epi = s0 * ref + s1 * vecs[0] + s2 * vecs[1] + s3 * vecs[2]
+    results = {}
+    for variant in ("site", "tile", "tile_tma", "auto"):
+        ctx.set_stencil_variant(variant)
+        ctx.apply_Q(y, x, -1.6)
+        got = ctx.unpack_spinor(y)
+        assert rel_l2(got, ref) <= TOL[32], (variant, rel_l2(got, ref))
+        results[variant] = got
+        out = ctx.new_spinor()
+        ctx.copy(out, d[1])
+        ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])   # out aliases v2, as in the Clenshaw step
+        assert rel_l2(ctx.unpack_spinor(out), ref_epi) <= TOL[32], variant
+    # cp.async and TMA prefetch feed the same arithmetic: bit-identical results
+    assert np.array_equal(results["tile"], results["tile_tma"])
+    # auto = the tiled kernel, except for the plain stencil with uncompressed links (the site-per-thread kernel is faster there)
+    assert np.array_equal(results["site" if recon == 18 else "tile"], results["auto"])
+    # worst site against the oracle, not only the norm
+    scale = np.abs(ref).max()
+    assert np.abs(results["tile"] - ref).max() <= (2e-5 if recon != 8 else 2e-4) * scale
+
+
+def test_variant_selection_rules():
+    import paper_1010_5636_b200 as nd
+
+    ctx, _ = make_context((8, 8, 8, 16), 32, 12)                     # x3 extent 16: no tiled kernel
+    assert ctx.get_stencil_variant() == "site"
+    with pytest.raises(nd.NDError) as e:
+        ctx.set_stencil_variant("tile")
+    assert e.value.code == -1
+    ctx64, _ = make_context((40, 8, 16, 32), 64, 12)                 # fp64: site-per-thread kernel
+    assert ctx64.get_stencil_variant() == "site"
+    with pytest.raises(nd.NDError):
+        ctx64.set_stencil_variant("tile_tma")
