@@ -142,6 +142,13 @@ ND_API int nd_set_lowmodes(nd_ctx* ctx, int l, const void* u_soa, const double* 
  * sequence as a CUDA graph cached on (out, in, work). */
 ND_API int nd_apply_sign(nd_ctx* ctx, void* out, const void* in, void* work, int use_graph);
 ND_API int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor, void* work, int use_graph);
+/* The same operators on nrhs right-hand sides at once (1 <= nrhs <= 16, nrhs * l <= 256): in, out = nrhs device spinors stored
+ * back to back, work = 3 * nrhs spinors.  Every launch of the sequence handles all right-hand sides (stencils: one grid row
+ * per source, the links shared through L1 / L2; projection: the low modes are streamed once for all sources), so small
+ * lattices - one source of 8^3x16 occupies a quarter of the machine - fill the GPU; per source the arithmetic is exactly that
+ * of nd_apply_sign / nd_apply_DN. */
+ND_API int nd_apply_sign_multi(nd_ctx* ctx, int nrhs, void* out, const void* in, void* work, int use_graph);
+ND_API int nd_apply_DN_multi(nd_ctx* ctx, int nrhs, void* out, const void* in, double prefactor, void* work, int use_graph);
 
 /* ------------------------------------------------------------------------------- massive operator and solver
  * nd_apply_DNm: the massive Neuberger-Dirac operator behind the bound (2.12) (R16)

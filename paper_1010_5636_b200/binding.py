@@ -50,6 +50,8 @@ SIGNATURES = {
     "nd_set_lowmodes": (_c_int, [_c_vp, _c_int, _c_vp, _pd]),
     "nd_apply_sign": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_int]),
     "nd_apply_DN": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_vp, _c_int]),
+    "nd_apply_sign_multi": (_c_int, [_c_vp, _c_int, _c_vp, _c_vp, _c_vp, _c_int]),
+    "nd_apply_DN_multi": (_c_int, [_c_vp, _c_int, _c_vp, _c_vp, _c_dbl, _c_vp, _c_int]),
     "nd_apply_DNm": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_vp, _c_int]),
     "nd_solve_DNm": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_dbl, _c_int, _c_vp, _pd, ctypes.POINTER(_c_int)]),
     "nd_solve_DNm_mixed": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_dbl, _c_dbl, _c_int, _c_int, _c_vp, _c_vp, _pd,
@@ -326,6 +328,18 @@ class Context:
         assert work.is_contiguous() and work.numel() >= 3 * 24 * self.V
         self._chk(self.lib.nd_apply_DN(self._h, out.data_ptr(), inp.data_ptr(), float(prefactor), work.data_ptr(),
                                        int(use_graph)))
+
+    def apply_sign_multi(self, out, inp, work, use_graph=False):
+        """out, inp: [nrhs, 24 V]; work: 3 * nrhs spinors."""
+        nrhs = inp.shape[0]
+        assert out.shape == inp.shape and out.is_contiguous() and inp.is_contiguous() and work.numel() >= 3 * nrhs * 24 * self.V
+        self._chk(self.lib.nd_apply_sign_multi(self._h, nrhs, out.data_ptr(), inp.data_ptr(), work.data_ptr(), int(use_graph)))
+
+    def apply_DN_multi(self, out, inp, prefactor, work, use_graph=False):
+        nrhs = inp.shape[0]
+        assert out.shape == inp.shape and out.is_contiguous() and inp.is_contiguous() and work.numel() >= 3 * nrhs * 24 * self.V
+        self._chk(self.lib.nd_apply_DN_multi(self._h, nrhs, out.data_ptr(), inp.data_ptr(), float(prefactor), work.data_ptr(),
+                                             int(use_graph)))
 
     def apply_DNm(self, out, inp, prefactor, mq, work, use_graph=False):
         assert work.is_contiguous() and work.numel() >= 3 * 24 * self.V

@@ -78,6 +78,7 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     for (int i = 0; i < 4; i++) ctx->tile_ctas_per_sm[i] = 0;
     ctx->tile_ok = ndi_tile_supported(ctx);
     ctx->stencil_variant = ND_STENCIL_AUTO;
+    ctx->dot_configured = false;
     // fp32 recon 18 is stored as 9 float2, everything else in 128-bit words: bytes = 4 * recon * V * prec/8
     ctx->gauge_bytes = (size_t)4 * recon * ctx->V * (prec / 8);
     cudaError_t e = cudaMalloc(&ctx->gauge, ctx->gauge_bytes);

@@ -2,6 +2,8 @@
 // projection kernels  w_k = <u_k, x>  and  y <- y + sum_k a_k u_k  (eq. 2.7 / 2.11).
 // All reductions accumulate in fp64 (both precisions): thread partials -> warp shuffle -> per-warp shared row ->
 // per-block partial -> second-stage kernel.  No atomics: results are bitwise reproducible run to run.
+#include <vector>
+
 #include "nd_internal.cuh"
 
 namespace {
@@ -70,62 +72,99 @@ __global__ void gamma5_kernel(typename Prec<T>::Vec* y, const typename Prec<T>::
 }
 
 // --------------------------------------------------------------------------------------- block dot product
-// partial[(j*l + k)*2 + {0,1}][block] = sum over this block's sites of conj(v_k) x_j ,  j < NX
-template <typename T, int NX>
-__global__ void __launch_bounds__(RED_THREADS) block_dot_kernel(double* __restrict__ partial, int l,
-                                                                const typename Prec<T>::Vec* __restrict__ v,
-                                                                const typename Prec<T>::Vec* __restrict__ x0,
-                                                                const typename Prec<T>::Vec* __restrict__ x1, long long V) {
-    extern __shared__ double sm[];   // [RED_WARPS][NX*l*2]
+// <v_k, x_c> for k < l vectors of a block and up to NC columns x_c given by pointer (eq. 2.7 / 2.11: V^dagger psi; the
+// eigen-solver's Gram matrices).  Both operands move through HBM exactly once:
+//   a CTA takes ranges of DOT_RANGE consecutive sites; the NC columns of the range are staged in shared memory ONCE, then
+//   the block's vectors are streamed: for every k each thread reads its sites of v_k (coalesced, each element of the block
+//   is read by exactly one thread of the grid), multiplies with the staged columns and accumulates in fp64 registers; one
+//   warp reduction per (k, column) and RANGE, accumulated per CTA in shared memory;
+//   partial[((c*l + k)*2 + {re,im})][cta]  ->  reduce_partials_kernel.  No atomics: bitwise reproducible.
+struct ColPtrs {
+    const void* p[8];
+};
+constexpr int DOT_SITES_PER_THREAD = 2;
+constexpr int DOT_RANGE = RED_THREADS * DOT_SITES_PER_THREAD;
+
+template <typename T, int NC>
+__global__ void __launch_bounds__(RED_THREADS) block_dot_cols_kernel(double* __restrict__ partial, int l, int nc,
+                                                                     const typename Prec<T>::Vec* __restrict__ v, ColPtrs cols, long long V) {
+    using Vec = typename Prec<T>::Vec;
+    constexpr int NV = Prec<T>::NV;
+    extern __shared__ __align__(16) unsigned char dsm[];
+    Vec* xs = reinterpret_cast<Vec*>(dsm);                                              // [NC][NV][DOT_RANGE]
+    double* acc = reinterpret_cast<double*>(dsm + (size_t)NC * NV * DOT_RANGE * sizeof(Vec));   // [nc*l*2] CTA totals
+    double* wred = acc + (size_t)2 * NC * l;                                            // [RED_WARPS][2*NC]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int row = NX * l * 2;
-    for (int i = threadIdx.x; i < RED_WARPS * row; i += blockDim.x) sm[i] = 0.0;
-    __syncthreads();
-    const long long nchunks = (V + blockDim.x - 1) / blockDim.x;
-    for (long long ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
-        const long long s = ch * blockDim.x + threadIdx.x;
-        const bool valid = s < V;
-        const long long sc = valid ? s : V - 1;
-        cx<T> a[NX][12];
-        load_site<T>(x0, V, sc, a[0]);
-        if (NX > 1) load_site<T>(x1, V, sc, a[NX - 1]);
-        if (!valid) {
+    for (int i = threadIdx.x; i < 2 * nc * l; i += blockDim.x) acc[i] = 0.0;
+    const long long nranges = (V + DOT_RANGE - 1) / DOT_RANGE;
+    for (long long rg = blockIdx.x; rg < nranges; rg += gridDim.x) {
+        const long long base = rg * DOT_RANGE;
+        __syncthreads();   // the previous range's columns are no longer read; acc initialised
+        for (int c = 0; c < nc; c++) {
+            const Vec* xc = reinterpret_cast<const Vec*>(cols.p[c]);
 #pragma unroll
-            for (int j = 0; j < NX; j++)
+            for (int p = 0; p < NV; p++)
 #pragma unroll
-                for (int i = 0; i < 12; i++) a[j][i] = {T(0), T(0)};
-        }
-        for (int k = 0; k < l; k++) {
-            cx<T> b[12];
-            load_site<T>(v + (long long)k * Prec<T>::NV * V, V, sc, b);
+                for (int j = 0; j < DOT_SITES_PER_THREAD; j++) {
+                    const long long s = base + j * RED_THREADS + threadIdx.x;
+                    Vec w;
+                    T* wr = reinterpret_cast<T*>(&w);
 #pragma unroll
-            for (int j = 0; j < NX; j++) {
-                double re = 0.0, im = 0.0;
-#pragma unroll
-                for (int i = 0; i < 12; i++) {
-                    // conj(b) * a, products in T (exact in fp64 for fp32 inputs would need widening: widen)
-                    const double br = (double)b[i].re, bi = (double)b[i].im, xr = (double)a[j][i].re, xi = (double)a[j][i].im;
-                    re = fma(br, xr, re);
-                    re = fma(bi, xi, re);
-                    im = fma(br, xi, im);
-                    im = fma(-bi, xr, im);
+                    for (int q = 0; q < (int)(sizeof(Vec) / sizeof(T)); q++) wr[q] = T(0);
+                    if (s < V) w = xc[p * V + s];
+                    xs[(c * NV + p) * DOT_RANGE + j * RED_THREADS + threadIdx.x] = w;
                 }
-                re = warp_sum(re);
-                im = warp_sum(im);
-                if (lane == 0) {
-                    sm[warp * row + (j * l + k) * 2] += re;
-                    sm[warp * row + (j * l + k) * 2 + 1] += im;
+        }
+        __syncthreads();
+        for (int k = 0; k < l; k++) {
+            const Vec* vk = v + (long long)k * NV * V;
+            double re[NC], im[NC];
+#pragma unroll
+            for (int c = 0; c < NC; c++) re[c] = im[c] = 0.0;
+#pragma unroll
+            for (int j = 0; j < DOT_SITES_PER_THREAD; j++) {
+                const long long s = base + j * RED_THREADS + threadIdx.x;
+                if (s < V) {
+                    cx<T> b[12];
+                    load_site<T>(vk, V, s, b);
+#pragma unroll
+                    for (int c = 0; c < NC; c++) {
+                        if (c < nc) {
+                            Vec w[NV];
+#pragma unroll
+                            for (int p = 0; p < NV; p++) w[p] = xs[(c * NV + p) * DOT_RANGE + j * RED_THREADS + threadIdx.x];
+                            cx<T> a[12];
+                            words_to_cx(w, a);
+#pragma unroll
+                            for (int i = 0; i < 12; i++) {
+                                const double br = (double)b[i].re, bi = (double)b[i].im, xr = (double)a[i].re, xi = (double)a[i].im;
+                                re[c] = fma(br, xr, re[c]);
+                                re[c] = fma(bi, xi, re[c]);
+                                im[c] = fma(br, xi, im[c]);
+                                im[c] = fma(-bi, xr, im[c]);
+                            }
+                        }
+                    }
                 }
             }
+#pragma unroll
+            for (int c = 0; c < NC; c++) {
+                re[c] = warp_sum(re[c]);
+                im[c] = warp_sum(im[c]);
+                if (lane == 0) { wred[warp * 2 * NC + 2 * c] = re[c]; wred[warp * 2 * NC + 2 * c + 1] = im[c]; }
+            }
+            __syncthreads();
+            if (threadIdx.x < 2 * nc) {
+                double t = 0.0;
+#pragma unroll
+                for (int w = 0; w < RED_WARPS; w++) t += wred[w * 2 * NC + threadIdx.x];
+                acc[((threadIdx.x >> 1) * l + k) * 2 + (threadIdx.x & 1)] += t;
+            }
+            __syncthreads();
         }
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < row; i += blockDim.x) {
-        double t = 0.0;
-#pragma unroll
-        for (int w = 0; w < RED_WARPS; w++) t += sm[w * row + i];
-        partial[(long long)i * gridDim.x + blockIdx.x] = t;
-    }
+    for (int i = threadIdx.x; i < 2 * nc * l; i += blockDim.x) partial[(long long)i * gridDim.x + blockIdx.x] = acc[i];
 }
 
 // out[i] = sum_b partial[i][b]; one block per i
@@ -179,64 +218,51 @@ __global__ void __launch_bounds__(RED_THREADS) block_axpy_kernel(typename Prec<T
     }
 }
 
-// ----------------------------------------------------------------------------------- grouped Gram / rotation
-// The eigen-solver needs X^dagger Y and X C for blocks of k vectors (lowmodes.cu).  Column by column (block_dot /
-// block_axpy) the block X is re-read k times.  These two kernels take NG columns at a time, so X is streamed k/NG times.
-//
-// gram: partial[((j*l + k)*2 + c)][block] = sum over the block's sites of conj(v_k) x_j, j < ng <= NG.  The loop over
-// k is OUTSIDE the loop over the CTA's sites: the NG x-columns of those sites are re-read from L1/L2, v_k is streamed
-// once, and the accumulators of one k fit in registers, so there is one warp reduction per k and not one per chunk.
-template <typename T, int NG>
-__global__ void __launch_bounds__(RED_THREADS) block_gram_kernel(double* __restrict__ partial, int l, int ng,
-                                                                 const typename Prec<T>::Vec* __restrict__ v,
-                                                                 const typename Prec<T>::Vec* __restrict__ x, long long V) {
-    __shared__ double sm[RED_WARPS][2 * NG];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long nchunks = (V + blockDim.x - 1) / blockDim.x;
-    for (int k = 0; k < l; k++) {
-        double re[NG], im[NG];
+// the same for NB right-hand sides at once (nd_apply_DN_multi): y_j, eta_j are batches (stride = one spinor), coef[(j*l + k)*2];
+// the block v is streamed once for all of them
+template <typename T, int NB, int MODE>
+__global__ void __launch_bounds__(RED_THREADS) block_axpy_batch_kernel(typename Prec<T>::Vec* y, int l, int nb, const double* __restrict__ coef,
+                                                                       const typename Prec<T>::Vec* __restrict__ v,
+                                                                       const typename Prec<T>::Vec* eta, T pa, T pb, long long V) {
+    extern __shared__ double sm[];   // [nb][2l]
+    for (int i = threadIdx.x; i < 2 * l * nb; i += blockDim.x) sm[i] = coef[i];
+    __syncthreads();
+    const long long bs = (long long)Prec<T>::NV * V;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < V; s += (long long)gridDim.x * blockDim.x) {
+        cx<T> c[NB][12];
 #pragma unroll
-        for (int j = 0; j < NG; j++) re[j] = im[j] = 0.0;
-        const typename Prec<T>::Vec* vk = v + (long long)k * Prec<T>::NV * V;
-        for (long long ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
-            const long long s = ch * blockDim.x + threadIdx.x;
-            if (s >= V) continue;
+        for (int j = 0; j < NB; j++)
+            if (j < nb) load_site<T>(y + j * bs, V, s, c[j]);
+        for (int k = 0; k < l; k++) {
             cx<T> b[12];
-            load_site<T>(vk, V, s, b);
+            load_site<T>(v + (long long)k * bs, V, s, b);
 #pragma unroll
-            for (int j = 0; j < NG; j++) {
-                if (j < ng) {
-                    cx<T> a[12];
-                    load_site<T>(x + (long long)j * Prec<T>::NV * V, V, s, a);
+            for (int j = 0; j < NB; j++)
+                if (j < nb) {
+                    const cx<T> a = {(T)sm[(j * l + k) * 2], (T)sm[(j * l + k) * 2 + 1]};
+#pragma unroll
+                    for (int i = 0; i < 12; i++) cfma(c[j][i], a, b[i]);
+                }
+        }
+#pragma unroll
+        for (int j = 0; j < NB; j++)
+            if (j < nb) {
+                if (MODE == 1) {
+                    cx<T> e[12];
+                    load_site<T>(eta + j * bs, V, s, e);
 #pragma unroll
                     for (int i = 0; i < 12; i++) {
-                        const double br = (double)b[i].re, bi = (double)b[i].im, xr = (double)a[i].re, xi = (double)a[i].im;
-                        re[j] = fma(br, xr, re[j]);
-                        re[j] = fma(bi, xi, re[j]);
-                        im[j] = fma(br, xi, im[j]);
-                        im[j] = fma(-bi, xr, im[j]);
+                        const T sg = (i < 6) ? T(1) : T(-1);
+                        c[j][i] = {fma(pa, e[i].re, pb * sg * c[j][i].re), fma(pa, e[i].im, pb * sg * c[j][i].im)};
                     }
                 }
+                store_site<T>(y + j * bs, V, s, c[j]);
             }
-        }
-#pragma unroll
-        for (int j = 0; j < NG; j++) {
-            re[j] = warp_sum(re[j]);
-            im[j] = warp_sum(im[j]);
-            if (lane == 0) { sm[warp][2 * j] = re[j]; sm[warp][2 * j + 1] = im[j]; }
-        }
-        __syncthreads();
-        if (threadIdx.x < 2 * ng) {
-            double t = 0.0;
-#pragma unroll
-            for (int w = 0; w < RED_WARPS; w++) t += sm[w][threadIdx.x];
-            const int j = threadIdx.x >> 1, c = threadIdx.x & 1;
-            partial[((long long)(j * l + k) * 2 + c) * gridDim.x + blockIdx.x] = t;
-        }
-        __syncthreads();
     }
 }
 
+// ------------------------------------------------------------------------------------------- block rotation
+// The eigen-solver needs X C for blocks of k vectors (lowmodes.cu): NG output columns at a time, so X is streamed k/NG times.
 // rotate: y_j = sum_{i < l} coef[j*l + i] v_i for j < ng <= NG output columns (y_j at y + j*NV*V), one pass over v
 template <typename T, int NG>
 __global__ void __launch_bounds__(RED_THREADS) block_rotate_kernel(typename Prec<T>::Vec* __restrict__ y, int l, int ng,
@@ -356,18 +382,37 @@ inline unsigned grid_for(long long n, int threads, int cap = ND_MAX_RED_BLOCKS) 
     return (unsigned)b;
 }
 
+// <v_k, x_c>, k < l, for nc columns (pointers) -> d_out[(c*l + k)*2 + {re, im}] (device), NC columns per pass over the block
 template <typename T>
-int block_dot_t(nd_ctx* ctx, int l, int nx, const void* v, const void* x0, const void* x1, double* d_out) {
+int block_dot_cols_t(nd_ctx* ctx, int l, const void* v, int nc, const void* const* cols, double* d_out) {
     using Vec = typename Prec<T>::Vec;
-    const unsigned blocks = grid_for(ctx->V, RED_THREADS);
-    const size_t smem = (size_t)RED_WARPS * nx * l * 2 * sizeof(double);
-    if (nx == 1)
-        block_dot_kernel<T, 1><<<blocks, RED_THREADS, smem, ctx->stream>>>(ctx->d_partial, l, (const Vec*)v, (const Vec*)x0, nullptr, ctx->V);
-    else
-        block_dot_kernel<T, 2><<<blocks, RED_THREADS, smem, ctx->stream>>>(ctx->d_partial, l, (const Vec*)v, (const Vec*)x0, (const Vec*)x1, ctx->V);
-    ND_LAUNCHED(ctx);
-    reduce_partials_kernel<<<nx * l * 2, RED_THREADS, 0, ctx->stream>>>(d_out, ctx->d_partial, (int)blocks);
-    ND_LAUNCHED(ctx);
+    // staged columns: NC * 24 reals * DOT_RANGE sites of shared memory (fp32: 24 KB, fp64: 48 KB per column)
+    constexpr int NCMAX = sizeof(T) == 4 ? 4 : 2;
+    auto smem_for = [](int NC, int ll) {
+        return (size_t)NC * Prec<T>::NV * DOT_RANGE * sizeof(Vec) + ((size_t)2 * NC * ll + (size_t)RED_WARPS * 2 * NC) * sizeof(double);
+    };
+    if (!ctx->dot_configured) {   // once per context (both precisions' instantiations are cheap to configure)
+        ND_CUDA(ctx, cudaFuncSetAttribute(block_dot_cols_kernel<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_for(1, ND_MAX_BLOCK_L)));
+        ND_CUDA(ctx, cudaFuncSetAttribute(block_dot_cols_kernel<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_for(2, ND_MAX_BLOCK_L)));
+        ND_CUDA(ctx, cudaFuncSetAttribute(block_dot_cols_kernel<T, NCMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_for(NCMAX, ND_MAX_BLOCK_L)));
+        ctx->dot_configured = true;
+    }
+    const long long nranges = (ctx->V + DOT_RANGE - 1) / DOT_RANGE;
+    for (int c0 = 0; c0 < nc; c0 += NCMAX) {
+        const int n = nc - c0 < NCMAX ? nc - c0 : NCMAX;
+        ColPtrs cp;
+        for (int i = 0; i < 8; i++) cp.p[i] = (i < n) ? cols[c0 + i] : nullptr;
+        // the partial-sum scratch holds ND_RESULT_DOUBLES x ND_MAX_RED_BLOCKS doubles: rows (2 l n) x CTAs must fit
+        long long cap = (long long)ND_RESULT_DOUBLES * ND_MAX_RED_BLOCKS / ((long long)2 * l * n);
+        if (cap > 8LL * ctx->num_sms) cap = 8LL * ctx->num_sms;
+        const unsigned blocks = (unsigned)(nranges < cap ? nranges : cap);
+        if (n == 1) block_dot_cols_kernel<T, 1><<<blocks, RED_THREADS, smem_for(1, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
+        else if (n == 2) block_dot_cols_kernel<T, 2><<<blocks, RED_THREADS, smem_for(2, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
+        else block_dot_cols_kernel<T, NCMAX><<<blocks, RED_THREADS, smem_for(NCMAX, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
+        ND_LAUNCHED(ctx);
+        reduce_partials_kernel<<<n * l * 2, RED_THREADS, 0, ctx->stream>>>(d_out + (size_t)2 * l * c0, ctx->d_partial, (int)blocks);
+        ND_LAUNCHED(ctx);
+    }
     return ND_OK;
 }
 
@@ -381,11 +426,16 @@ int ndi_read_result(nd_ctx* ctx, const double* d_src, double* h_dst, int n) {
     return ND_OK;
 }
 
+int ndi_block_dot_cols_dev(nd_ctx* ctx, int l, const void* v, int nc, const void* const* cols, double* d_out) {
+    return (ctx->prec == 32) ? block_dot_cols_t<float>(ctx, l, v, nc, cols, d_out) : block_dot_cols_t<double>(ctx, l, v, nc, cols, d_out);
+}
 int ndi_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out) {
-    return (ctx->prec == 32) ? block_dot_t<float>(ctx, l, 1, v, x, nullptr, d_out) : block_dot_t<double>(ctx, l, 1, v, x, nullptr, d_out);
+    const void* cols[1] = {x};
+    return ndi_block_dot_cols_dev(ctx, l, v, 1, cols, d_out);
 }
 int ndi_block_dot2_dev(nd_ctx* ctx, int l, const void* v, const void* x0, const void* x1, double* d_out) {
-    return (ctx->prec == 32) ? block_dot_t<float>(ctx, l, 2, v, x0, x1, d_out) : block_dot_t<double>(ctx, l, 2, v, x0, x1, d_out);
+    const void* cols[2] = {x0, x1};
+    return ndi_block_dot_cols_dev(ctx, l, v, 2, cols, d_out);
 }
 // y <- y + sum_k coef_k v_k (mode 0) or the D_N assembly (mode 1); coef on the device
 int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pa,
@@ -426,18 +476,29 @@ int ndi_block_resid(nd_ctx* ctx, int k, const void* x, const void* y, const doub
 // G[k][j] = <v_k, x_j>, k < l, j < nx, into d_out[(j*l + k)*2 + {re, im}] (device); x_j at x + j*spinor_bytes
 int ndi_block_gram_dev(nd_ctx* ctx, int l, const void* v, int nx, const void* x, double* d_out) {
     const size_t sb = nd_spinor_bytes(ctx);
-    const int NG = ctx->prec == 32 ? 8 : 4;
-    // the partial-sum scratch holds ND_RESULT_DOUBLES x ND_MAX_RED_BLOCKS doubles: rows (2 l NG) x blocks must fit
-    long long cap = (long long)ND_RESULT_DOUBLES * ND_MAX_RED_BLOCKS / ((long long)2 * l * NG);
-    if (cap > 4 * ctx->num_sms) cap = 4 * ctx->num_sms;
-    const unsigned blocks = grid_for(ctx->V, RED_THREADS, (int)cap);
-    for (int j0 = 0; j0 < nx; j0 += NG) {
-        const int ng = nx - j0 < NG ? nx - j0 : NG;
-        const char* xj = (const char*)x + (size_t)j0 * sb;
-        if (ctx->prec == 32) block_gram_kernel<float, 8><<<blocks, RED_THREADS, 0, ctx->stream>>>(ctx->d_partial, l, ng, (const float4*)v, (const float4*)xj, ctx->V);
-        else block_gram_kernel<double, 4><<<blocks, RED_THREADS, 0, ctx->stream>>>(ctx->d_partial, l, ng, (const double2*)v, (const double2*)xj, ctx->V);
-        ND_LAUNCHED(ctx);
-        reduce_partials_kernel<<<ng * l * 2, RED_THREADS, 0, ctx->stream>>>(d_out + (size_t)2 * l * j0, ctx->d_partial, (int)blocks);
+    std::vector<const void*> cols(nx);
+    for (int j = 0; j < nx; j++) cols[j] = (const char*)x + (size_t)j * sb;
+    return ndi_block_dot_cols_dev(ctx, l, v, nx, cols.data(), d_out);
+}
+// batched block axpy (nb right-hand sides, coef[(j*l + k)*2] on the device); mode as ndi_block_axpy_dev
+int ndi_block_axpy_batch_dev(nd_ctx* ctx, int l, int nb, const double* d_coef, const void* v, void* y, int mode, const void* eta,
+                             double pa, double pb) {
+    const size_t sb = nd_spinor_bytes(ctx);
+    const int NB = ctx->prec == 32 ? 4 : 2;
+    const unsigned blocks = grid_for(ctx->V, RED_THREADS, 1 << 30);
+    for (int j0 = 0; j0 < nb; j0 += NB) {
+        const int n = nb - j0 < NB ? nb - j0 : NB;
+        char* yj = (char*)y + (size_t)j0 * sb;
+        const char* ej = eta ? (const char*)eta + (size_t)j0 * sb : nullptr;
+        const double* cj = d_coef + (size_t)2 * l * j0;
+        const size_t smem = (size_t)2 * (l > 0 ? l : 1) * n * sizeof(double);
+        if (ctx->prec == 32) {
+            if (mode == 0) block_axpy_batch_kernel<float, 4, 0><<<blocks, RED_THREADS, smem, ctx->stream>>>((float4*)yj, l, n, cj, (const float4*)v, nullptr, 0.f, 0.f, ctx->V);
+            else block_axpy_batch_kernel<float, 4, 1><<<blocks, RED_THREADS, smem, ctx->stream>>>((float4*)yj, l, n, cj, (const float4*)v, (const float4*)ej, (float)pa, (float)pb, ctx->V);
+        } else {
+            if (mode == 0) block_axpy_batch_kernel<double, 2, 0><<<blocks, RED_THREADS, smem, ctx->stream>>>((double2*)yj, l, n, cj, (const double2*)v, nullptr, 0.0, 0.0, ctx->V);
+            else block_axpy_batch_kernel<double, 2, 1><<<blocks, RED_THREADS, smem, ctx->stream>>>((double2*)yj, l, n, cj, (const double2*)v, (const double2*)ej, pa, pb, ctx->V);
+        }
         ND_LAUNCHED(ctx);
     }
     return ND_OK;

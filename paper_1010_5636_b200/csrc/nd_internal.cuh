@@ -25,6 +25,7 @@ struct nd_graph_entry {
     double pa, pb;       // out = pa*in + pb*gamma5 sign(Q) in
     cudaGraphExec_t exec;
     long long nodes;     // kernel launches one replay stands for
+    int nrhs;
 };
 
 struct nd_ctx {
@@ -59,6 +60,7 @@ struct nd_ctx {
     int hop_max_sites;  // lattices below this volume use the hop-parallel stencil (wilson.cu)
     int tile_lb[3];     // stencil CTA tile: log2 extents along x1, x2, x3
     int tile_threads;   // sites per tile (0: linear mapping)
+    bool dot_configured;        // block_dot_cols_kernel shared-memory attributes set
     bool tile_ok;               // the tiled marching stencil (wilson_tile.cu) takes this lattice
     int stencil_variant;        // ND_STENCIL_* (nd_set_stencil_variant)
     int tile_ctas_per_sm[4];    // resident CTAs per SM of the tiled kernel ({cp.async, TMA} x {plain, fused}), 0 = not queried yet
@@ -67,6 +69,7 @@ struct nd_ctx {
 
 constexpr int ND_MAX_BLOCK_L = 256;     // max vectors in a block dot / block axpy
 constexpr int ND_MAX_RED_BLOCKS = 1184; // 8 x 148
+constexpr int ND_MAX_RHS = 16;          // right-hand sides of one nd_apply_*_multi call
 
 int nd_fail(nd_ctx* ctx, int code, const char* fmt, ...);
 int nd_cuda_check(nd_ctx* ctx, cudaError_t e, const char* what);
@@ -156,7 +159,12 @@ int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, doub
 bool ndi_tile_supported(const nd_ctx* ctx);
 int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                      const void* v2, double s3, const void* v3);
+int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
+                      double s2, const void* v2, double s3, const void* v3);
 int ndi_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out);   // d_out: 2l doubles (device)
+int ndi_block_dot_cols_dev(nd_ctx* ctx, int l, const void* v, int nc, const void* const* cols, double* d_out);   // d_out[(c*l+k)*2+ri]
+int ndi_block_axpy_batch_dev(nd_ctx* ctx, int l, int nb, const double* d_coef, const void* v, void* y, int mode, const void* eta,
+                             double pa, double pb);
 int ndi_block_dot2_dev(nd_ctx* ctx, int l, const void* v, const void* x0, const void* x1, double* d_out);  // 4l doubles
 int ndi_block_axpy_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, void* y, int mode, const void* eta, double pa,
                        double pb);   // mode 1: y <- pa*eta + pb*gamma5(y + sum_k a_k v_k)

@@ -28,17 +28,19 @@ __global__ void scale_copy_kernel(typename Prec<T>::Vec* __restrict__ y, const t
     }
 }
 
-// coef_k = sign(nu_k) <u_k,eta> - <u_k,chi>   (dots = [<u,eta> (2l) | <u,chi> (2l)])
-__global__ void lowmode_coef_kernel(double* __restrict__ coef, const double* __restrict__ dots, const double* __restrict__ nu, int l) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= l) return;
+// coef_jk = sign(nu_k) <u_k,eta_j> - <u_k,chi_j> for nb right-hand sides
+// (dots = [<u,eta_0> (2l) | ... | <u,eta_{nb-1}> | <u,chi_0> (2l) | ... | <u,chi_{nb-1}>], coef[(j*l + k)*2])
+__global__ void lowmode_coef_kernel(double* __restrict__ coef, const double* __restrict__ dots, const double* __restrict__ nu, int l, int nb) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= l * nb) return;
+    const int k = i % l;
     const double sg = (nu[k] > 0.0) ? 1.0 : ((nu[k] < 0.0) ? -1.0 : 0.0);
-    coef[2 * k] = sg * dots[2 * k] - dots[2 * l + 2 * k];
-    coef[2 * k + 1] = sg * dots[2 * k + 1] - dots[2 * l + 2 * k + 1];
+    coef[2 * i] = sg * dots[2 * i] - dots[2 * (l * nb + i)];
+    coef[2 * i + 1] = sg * dots[2 * i + 1] - dots[2 * (l * nb + i) + 1];
 }
 
-int scale_copy(nd_ctx* ctx, void* y, const void* x, double a) {
-    const long long nwords = ctx->V * (ctx->prec == 32 ? 6 : 12);
+int scale_copy(nd_ctx* ctx, void* y, const void* x, double a, int nb) {
+    const long long nwords = (long long)nb * ctx->V * (ctx->prec == 32 ? 6 : 12);
     long long b = (nwords + 255) / 256;
     if (ctx->prec == 32) scale_copy_kernel<float><<<(unsigned)b, 256, 0, ctx->stream>>>((float4*)y, (const float4*)x, (float)a, nwords);
     else scale_copy_kernel<double><<<(unsigned)b, 256, 0, ctx->stream>>>((double2*)y, (const double2*)x, a, nwords);
@@ -46,9 +48,10 @@ int scale_copy(nd_ctx* ctx, void* y, const void* x, double a) {
     return ND_OK;
 }
 
-// kind 0: out = sign(Q) in ; kind 1: out = prefactor (in + gamma5 sign(Q) in)
-int enqueue_sign(nd_ctx* ctx, void* out, const void* eta, void* work, int kind, double pa, double pb) {
-    const size_t sb = nd_spinor_bytes(ctx);
+// kind 0: out = sign(Q) in ; kind 1: out = pa in + pb gamma5 sign(Q) in ; for nb right-hand sides stored back to back
+// (out, eta: nb spinors; work: 3 nb spinors): every launch of the sequence handles all of them (stencils: blockIdx.y = rhs)
+int enqueue_sign(nd_ctx* ctx, int nb, void* out, const void* eta, void* work, int kind, double pa, double pb) {
+    const size_t sb = nd_spinor_bytes(ctx) * (size_t)nb;
     char* bA = (char*)work;
     char* bB = bA + sb;
     char* tmp = bB + sb;
@@ -59,55 +62,65 @@ int enqueue_sign(nd_ctx* ctx, void* out, const void* eta, void* work, int kind, 
     const double beta = -(1.0 + ctx->eps) / (1.0 - ctx->eps);
     int rc;
     if (n == 0) {
-        rc = ndi_apply_Q(ctx, out, eta, m, true, c[0] / ctx->qnorm, 0, nullptr, 0, nullptr, 0, nullptr);
+        rc = ndi_apply_Q_batch(ctx, nb, out, eta, m, true, c[0] / ctx->qnorm, 0, nullptr, 0, nullptr, 0, nullptr);
         if (rc != ND_OK) return rc;
     } else {
-        rc = scale_copy(ctx, bA, eta, c[n]);   // b_n = c_n eta ; b_{n+1} = 0 is never materialised
+        rc = scale_copy(ctx, bA, eta, c[n], nb);   // b_n = c_n eta ; b_{n+1} = 0 is never materialised
         if (rc != ND_OK) return rc;
         for (int k = n - 1; k >= 0; k--) {
             // tmp = Q b_{k+1};   b_k = f*(alpha Q tmp + beta b_{k+1}) - b_{k+2} + c_k eta,  f = 2 (k >= 1) or 1 (k = 0)
-            rc = ndi_apply_Q(ctx, tmp, bA, m, false, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+            rc = ndi_apply_Q_batch(ctx, nb, tmp, bA, m, false, 1, 0, nullptr, 0, nullptr, 0, nullptr);
             if (rc != ND_OK) return rc;
             const double f = (k >= 1) ? 2.0 : 1.0;
             const double s2 = (k == n - 1) ? 0.0 : -1.0;
-            rc = ndi_apply_Q(ctx, bB, tmp, m, true, f * alpha, f * beta, bA, s2, bB, c[k], eta);
+            rc = ndi_apply_Q_batch(ctx, nb, bB, tmp, m, true, f * alpha, f * beta, bA, s2, bB, c[k], eta);
             if (rc != ND_OK) return rc;
             char* t = bA; bA = bB; bB = t;
         }
         // bA = P eta ;  chi = Q P eta / qnorm
-        rc = ndi_apply_Q(ctx, out, bA, m, true, 1.0 / ctx->qnorm, 0, nullptr, 0, nullptr, 0, nullptr);
+        rc = ndi_apply_Q_batch(ctx, nb, out, bA, m, true, 1.0 / ctx->qnorm, 0, nullptr, 0, nullptr, 0, nullptr);
         if (rc != ND_OK) return rc;
     }
     const int l = ctx->l;
     if (l > 0) {
-        rc = ndi_block_dot2_dev(ctx, l, ctx->u, eta, out, ctx->d_result);
+        // one pass over the modes for <u_k,eta_j> and <u_k,chi_j> of all right-hand sides
+        const size_t s1 = nd_spinor_bytes(ctx);
+        const void* cols[2 * ND_MAX_RHS];
+        for (int j = 0; j < nb; j++) {
+            cols[j] = (const char*)eta + (size_t)j * s1;
+            cols[nb + j] = (const char*)out + (size_t)j * s1;
+        }
+        rc = ndi_block_dot_cols_dev(ctx, l, ctx->u, 2 * nb, cols, ctx->d_result);
         if (rc != ND_OK) return rc;
-        lowmode_coef_kernel<<<(l + 63) / 64, 64, 0, ctx->stream>>>(ctx->d_coef, ctx->d_result, ctx->d_nu, l);
+        lowmode_coef_kernel<<<(l * nb + 63) / 64, 64, 0, ctx->stream>>>(ctx->d_coef, ctx->d_result, ctx->d_nu, l, nb);
         ND_LAUNCHED(ctx);
     }
     if (l > 0 || kind == 1) {
-        rc = ndi_block_axpy_dev(ctx, l, ctx->d_coef, ctx->u, out, kind, eta, pa, pb);
+        rc = (nb == 1) ? ndi_block_axpy_dev(ctx, l, ctx->d_coef, ctx->u, out, kind, eta, pa, pb)
+                       : ndi_block_axpy_batch_dev(ctx, l, nb, ctx->d_coef, ctx->u, out, kind, eta, pa, pb);
         if (rc != ND_OK) return rc;
     }
     return ND_OK;
 }
 
-int apply_sign_impl(nd_ctx* ctx, void* out, const void* in, void* work, int kind, double pa, double pb, int use_graph) {
+int apply_sign_impl(nd_ctx* ctx, int nb, void* out, const void* in, void* work, int kind, double pa, double pb, int use_graph) {
     if (!ctx) return ND_ERR_BAD_ARG;
     if (!out || !in || !work || out == in) return nd_fail(ctx, ND_ERR_BAD_ARG, "apply_sign/DN: null or aliased argument");
+    if (nb < 1 || nb > ND_MAX_RHS || 4 * nb * (ctx->l > 0 ? ctx->l : 1) > ND_RESULT_DOUBLES || 2 * nb * ctx->l > 2 * ND_MAX_BLOCK_L)
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "apply_sign/DN: 1 <= nrhs <= %d and nrhs * l <= %d", ND_MAX_RHS, ND_MAX_BLOCK_L);
     if (!ctx->gauge_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_sign/DN: gauge field not set");
     if (!ctx->poly_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_sign/DN: polynomial not set (nd_set_sign_poly)");
     ND_CUDA(ctx, cudaSetDevice(ctx->device));
-    if (!use_graph || ctx->stream == nullptr) return enqueue_sign(ctx, out, in, work, kind, pa, pb);
+    if (!use_graph || ctx->stream == nullptr) return enqueue_sign(ctx, nb, out, in, work, kind, pa, pb);
     for (auto& g : ctx->graphs)
-        if (g.out == out && g.in == in && g.work == work && g.kind == kind && g.pa == pa && g.pb == pb) {
+        if (g.out == out && g.in == in && g.work == work && g.kind == kind && g.pa == pa && g.pb == pb && g.nrhs == nb) {
             ND_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
             ctx->launches += g.nodes;
             return ND_OK;
         }
     const long long before = ctx->launches;
     ND_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
-    int rc = enqueue_sign(ctx, out, in, work, kind, pa, pb);
+    int rc = enqueue_sign(ctx, nb, out, in, work, kind, pa, pb);
     cudaGraph_t graph = nullptr;
     cudaError_t e = cudaStreamEndCapture(ctx->stream, &graph);
     const long long nodes = ctx->launches - before;
@@ -118,7 +131,7 @@ int apply_sign_impl(nd_ctx* ctx, void* out, const void* in, void* work, int kind
     }
     ND_CUDA(ctx, e);
     nd_graph_entry g;
-    g.out = out; g.in = in; g.work = work; g.kind = kind; g.pa = pa; g.pb = pb; g.exec = nullptr; g.nodes = nodes;
+    g.out = out; g.in = in; g.work = work; g.kind = kind; g.pa = pa; g.pb = pb; g.exec = nullptr; g.nodes = nodes; g.nrhs = nb;
     e = cudaGraphInstantiate(&g.exec, graph, 0);
     cudaGraphDestroy(graph);
     ND_CUDA(ctx, e);
@@ -132,7 +145,7 @@ int apply_sign_impl(nd_ctx* ctx, void* out, const void* in, void* work, int kind
 }  // namespace
 
 int ndi_apply_DNm(nd_ctx* ctx, void* out, const void* in, double pa, double pb, void* work, int use_graph) {
-    return apply_sign_impl(ctx, out, in, work, 1, pa, pb, use_graph);
+    return apply_sign_impl(ctx, 1, out, in, work, 1, pa, pb, use_graph);
 }
 
 // --------------------------------------------------------------------------------------------------- C ABI
@@ -210,8 +223,14 @@ extern "C" int nd_set_lowmodes(nd_ctx* ctx, int l, const void* u_soa, const doub
 }
 
 extern "C" int nd_apply_sign(nd_ctx* ctx, void* out, const void* in, void* work, int use_graph) {
-    return apply_sign_impl(ctx, out, in, work, 0, 0.0, 0.0, use_graph);
+    return apply_sign_impl(ctx, 1, out, in, work, 0, 0.0, 0.0, use_graph);
 }
 extern "C" int nd_apply_DN(nd_ctx* ctx, void* out, const void* in, double prefactor, void* work, int use_graph) {
-    return apply_sign_impl(ctx, out, in, work, 1, prefactor, prefactor, use_graph);
+    return apply_sign_impl(ctx, 1, out, in, work, 1, prefactor, prefactor, use_graph);
+}
+extern "C" int nd_apply_sign_multi(nd_ctx* ctx, int nrhs, void* out, const void* in, void* work, int use_graph) {
+    return apply_sign_impl(ctx, nrhs, out, in, work, 0, 0.0, 0.0, use_graph);
+}
+extern "C" int nd_apply_DN_multi(nd_ctx* ctx, int nrhs, void* out, const void* in, double prefactor, void* work, int use_graph) {
+    return apply_sign_impl(ctx, nrhs, out, in, work, 1, prefactor, prefactor, use_graph);
 }

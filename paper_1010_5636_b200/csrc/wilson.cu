@@ -54,7 +54,12 @@ __global__ void __launch_bounds__(Q_THREADS, q_min_blocks<T>()) wilson_Q_kernel(
                                                        const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, Geom G,
                                                        T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2,
                                                        const typename Prec<T>::Vec* v2, T s3,
-                                                       const typename Prec<T>::Vec* v3) {
+                                                       const typename Prec<T>::Vec* v3, long long batch_stride) {
+    {   // blockIdx.y = right-hand side of a batch (nd_apply_DN_multi): every field pointer moves on by one spinor
+        const long long off = (long long)blockIdx.y * batch_stride;
+        out += off; in += off;
+        if (EPI) { if (v1) v1 += off; if (v2) v2 += off; if (v3) v3 += off; }
+    }
     long long s;
     int x0, x1, x2, x3;
     if (G.nt[2] == 0) {
@@ -141,10 +146,15 @@ __global__ void __launch_bounds__(256) wilson_Q_hop_kernel(typename Prec<T>::Vec
                                                            const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, Geom G,
                                                            T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2,
                                                            const typename Prec<T>::Vec* v2, T s3,
-                                                           const typename Prec<T>::Vec* v3) {
+                                                           const typename Prec<T>::Vec* v3, long long batch_stride) {
     using Vec = typename Prec<T>::Vec;
     constexpr int NV = Prec<T>::NV;
     constexpr int W = 24 / NV;   // reals per 128-bit word
+    {
+        const long long off = (long long)blockIdx.y * batch_stride;
+        out += off; in += off;
+        if (EPI) { if (v1) v1 += off; if (v2) v2 += off; if (v3) v3 += off; }
+    }
     __shared__ T red[8][24][32];
     const int lane = threadIdx.x, hop = threadIdx.y;
     const long long s = (long long)blockIdx.x * 32 + lane;
@@ -214,7 +224,7 @@ __global__ void __launch_bounds__(256) wilson_Q_hop_kernel(typename Prec<T>::Vec
 
 template <typename T, int RECON>
 int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
-             const void* v2, double s3, const void* v3) {
+             const void* v2, double s3, const void* v3, int nrhs) {
     using Vec = typename Prec<T>::Vec;
     using LVec = typename LinkLayout<T, RECON>::LVec;
     Geom G;
@@ -224,39 +234,41 @@ int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double 
     G.S1 = (long long)G.L2 * G.L3;
     G.S0 = (long long)G.L1 * G.L2 * G.L3;
     G.bc = ctx->bc;
+    const long long bstride = (long long)Prec<T>::NV * ctx->V;   // one spinor, in 128-bit words
     if (ctx->V < (long long)ctx->hop_max_sites) {
         // fewer sites than lanes on the chip: one warp per hop (latency-bound regime, BASELINE config 3)
-        const unsigned nb = (unsigned)((ctx->V + 31) / 32);
+        const dim3 nb((unsigned)((ctx->V + 31) / 32), (unsigned)nrhs, 1);
         const dim3 tb(32, 8, 1);
         if (epi)
             wilson_Q_hop_kernel<T, RECON, true><<<nb, tb, 0, ctx->stream>>>(
                 (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(s0), T(s1), (const Vec*)v1, T(s2),
-                (const Vec*)v2, T(s3), (const Vec*)v3);
+                (const Vec*)v2, T(s3), (const Vec*)v3, bstride);
         else
             wilson_Q_hop_kernel<T, RECON, false><<<nb, tb, 0, ctx->stream>>>(
                 (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(1), T(0), nullptr, T(0), nullptr, T(0),
-                nullptr);
+                nullptr, bstride);
         ND_LAUNCHED(ctx);
         return ND_OK;
     }
     // 128 threads per CTA; small lattices get smaller CTAs so that every SM has work
     int threads = 128;
     while (threads > 32 && ctx->V / threads < 2 * ctx->num_sms) threads /= 2;
-    unsigned blocks = (unsigned)((ctx->V + threads - 1) / threads);
+    unsigned blocks1 = (unsigned)((ctx->V + threads - 1) / threads);
     for (int i = 0; i < 3; i++) { G.lb[i] = ctx->tile_lb[i]; G.nt[i] = 0; }
     if (ctx->tile_threads > 0 && ctx->tile_threads <= Q_THREADS && ctx->V / ctx->tile_threads >= 2 * ctx->num_sms) {
         threads = ctx->tile_threads;
-        blocks = (unsigned)G.L0;
-        for (int i = 0; i < 3; i++) { G.nt[i] = ctx->dims[i + 1] >> G.lb[i]; blocks *= (unsigned)G.nt[i]; }
+        blocks1 = (unsigned)G.L0;
+        for (int i = 0; i < 3; i++) { G.nt[i] = ctx->dims[i + 1] >> G.lb[i]; blocks1 *= (unsigned)G.nt[i]; }
     }
+    const dim3 blocks(blocks1, (unsigned)nrhs, 1);
     if (epi)
         wilson_Q_kernel<T, RECON, true><<<blocks, threads, 0, ctx->stream>>>(
             (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(s0), T(s1), (const Vec*)v1, T(s2),
-            (const Vec*)v2, T(s3), (const Vec*)v3);
+            (const Vec*)v2, T(s3), (const Vec*)v3, bstride);
     else
         wilson_Q_kernel<T, RECON, false><<<blocks, threads, 0, ctx->stream>>>(
             (Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(1), T(0), nullptr, T(0), nullptr, T(0),
-            nullptr);
+            nullptr, bstride);
     ND_LAUNCHED(ctx);
     return ND_OK;
 }
@@ -265,7 +277,15 @@ int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double 
 
 int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
                 double s2, const void* v2, double s3, const void* v3) {
+    return ndi_apply_Q_batch(ctx, 1, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+}
+
+// the same stencil on nrhs right-hand sides stored back to back (out, in and every v_i are batches of nrhs spinors): one
+// launch with blockIdx.y = right-hand side; the links are shared through L1 / L2
+int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
+                      double s2, const void* v2, double s3, const void* v3) {
     if (!ctx) return ND_ERR_BAD_ARG;
+    if (nrhs < 1 || nrhs > 65535) return nd_fail(ctx, ND_ERR_BAD_ARG, "apply_Q: bad number of right-hand sides");
     if (!out || !in || out == in) return nd_fail(ctx, ND_ERR_BAD_ARG, "apply_Q: out/in null or aliased");
     if (!ctx->gauge_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_Q: gauge field not set");
     if (s1 == 0.0) v1 = nullptr;
@@ -278,8 +298,17 @@ int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, doub
     // uncompressed recon-18 links (64-bit words in fp32) only the fused-epilogue variant wins (224 vs 199 us plain, 252 vs 276 us fused)
     const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->recon != 18 || epi))
                                                                 : (ctx->stencil_variant != ND_STENCIL_SITE);
-    if (tile) return ndi_apply_Q_tile(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
-#define ND_DISPATCH(T, R) return launch_Q<T, R>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3)
+    if (tile) {   // large lattices: one launch per right-hand side already fills the machine
+        const size_t sb = nd_spinor_bytes(ctx);
+        for (int j = 0; j < nrhs; j++) {
+            const size_t o = (size_t)j * sb;
+            int rc = ndi_apply_Q_tile(ctx, (char*)out + o, (const char*)in + o, m, epi, s0, s1, v1 ? (const char*)v1 + o : nullptr, s2,
+                                      v2 ? (const char*)v2 + o : nullptr, s3, v3 ? (const char*)v3 + o : nullptr);
+            if (rc != ND_OK) return rc;
+        }
+        return ND_OK;
+    }
+#define ND_DISPATCH(T, R) return launch_Q<T, R>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3, nrhs)
     if (ctx->prec == 32) {
         if (ctx->recon == 18) ND_DISPATCH(float, 18);
         if (ctx->recon == 12) ND_DISPATCH(float, 12);
