@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py - the driver's measurement contract for the B200-native Wilson-Dirac / Neuberger-Dirac hot path.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference] [--quick]
 
 ONE step = one pass of the whole hot path over one source field on the
 BASELINE.json headline lattice 32^3x64 (config index 2: Haar-random SU(3) links, Gaussian source, m = -1.6):
@@ -10,17 +10,22 @@ one application of the Neuberger-Dirac operator  D_N eta = c (eta + gamma5 sign(
 assembly), the low-mode projection (a7 block dot / block axpy, a9 BLAS-1 reductions) and the D_N epilogue (a8).
 The layout step a1 (pack / unpack) is inside the `e2e` leg, which runs the same step from pinned HOST buffers.
 
-metric  = Wilson-Dirac GFLOP/s at the conventional 1320 flop per site per stencil application (BASELINE.json),
-          value = 1320 * V * (2n+1) * steps * n_gpus / time; D_N applications per second are reported alongside.
-roofline = the dominant kernel (the Q stencil), timed alone with CUDA events on the launching stream in the same
-          run, against the measured HBM copy peak of MEASURED_PEAKS.json (fp32 and fp64; the JSON's `roofline` is the
-          line's dtype, `q_kernel` holds every variant).
+metric   = Wilson-Dirac GFLOP/s at the conventional 1320 flop per site per stencil application (BASELINE.json),
+           value = 1320 * V * (2n+1) * steps * n_gpus / time; D_N applications per second and tau = time per Clenshaw
+           iteration per site (the paper's normalisation) are reported alongside.
+roofline = the dominant kernel (the Q stencil), timed alone with CUDA events on the launching stream in the same run
+           (median of 5 batches, clocks sampled meanwhile), against the measured HBM copy peak of MEASURED_PEAKS.json;
+           `q_kernel` holds every precision x recon variant and, for fp32, the stencil variants against each other.
+layout   = a1 alone: pack / unpack / link compression, GB/s over AoS + SoA bytes.
+configs  = the other timed BASELINE.json configurations, driver-run in the same line: index 1 (1000 back-to-back Q on
+           16^3x32, fp32 + fp64 x recon 12 / 8), index 3 (D_N on 8^3x16, fp64, about 20 modes from the library's
+           eigen-solver) and index 4 (D_N on 16^3x32, fp32, about 50 modes, degree 200, eigen-solve timed).
 cpu_baseline / --impl reference = the CPU oracle (oracle/, plain C + numpy, as it stands) on the host cores on a
-          bounded sample of the same recipe.
+           bounded sample of the same workload.
 
-Multi-GPU (DESIGN.md section 9): the path is single-GPU in the paper ("no communication necessary", PAPER.md:L52);
-`--gpus N` under torchrun runs N independent replicas (one lattice per GPU, different sources), no data-path
-collective, scaling = weak.  Timing: barrier + synchronize, CUDA events, max over ranks.
+Multi-GPU: `--gpus N` runs N independent replicas (one lattice per GPU, different sources), no
+data-path collective, scaling = weak; when not started by torchrun it starts the N ranks itself.  Timing: barrier +
+synchronize, CUDA events, max over ranks.
 """
 import argparse
 import json
@@ -40,6 +45,7 @@ FLOP_PER_SITE = 1320           # BASELINE.json metric convention
 METRIC = "Wilson-Dirac GFLOP/s (1320 flop/site)"
 M_KERNEL = -1.6                # kernel mass m = -rho (BASELINE.json configs 2-5)
 RHO = 1.6
+QNORM = abs(4.0 + M_KERNEL) + 4.0
 
 
 # ------------------------------------------------------------------------------------------------ helpers
@@ -58,24 +64,32 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def load_traffic(kernel_key):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+def load_traffic(kernel, lattice, prec, recon):
+    """DRAM bytes per launch (ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum) of `kernel` on `lattice` from
+    the committed capture table profiles/q_kernel_dram_traffic.csv, or None when there is no capture of exactly this
+    kernel / lattice / precision / recon."""
     p = os.path.join(ROOT, "profiles", "q_kernel_dram_traffic.csv")
     if not os.path.exists(p):
         return None
     with open(p) as f:
         for line in f:
-            parts = [s.strip() for s in line.split(",")]
-            if len(parts) >= 2 and parts[0] == kernel_key:
+            f_ = [s.strip() for s in line.split(",")]
+            if len(f_) >= 5 and f_[0] == kernel and f_[1] == lattice and f_[2] == str(prec) and f_[3] == str(recon):
                 try:
-                    return float(parts[1])
+                    return float(f_[4])
                 except ValueError:
                     return None
     return None
 
 
+def stencil_kernel_name(variant, sites):
+    if variant in ("tile", "tile_tma"):
+        return "wilson_Q_tile_kernel"
+    return "wilson_Q_hop_kernel" if sites < 16384 else "wilson_Q_kernel"
+
+
 class ClockSampler:
-    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+    """Samples nvidia-smi clocks / throttle reasons every 200 ms while a timed region runs."""
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
               "clocks_event_reasons.sw_power_cap")
@@ -93,9 +107,10 @@ class ClockSampler:
                  "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
-            return
+            return self
         self.thread = threading.Thread(target=self._read, daemon=True)
         self.thread.start()
+        return self
 
     def _read(self):
         for line in self.proc.stdout:
@@ -156,10 +171,29 @@ def whole_job_value(units_per_rank, world, ms):
     return units_per_rank * world / (ms * 1e-3)
 
 
+def spawn_command(argv, gpus, port):
+    """The command line that starts `gpus` ranks of this script on one node (used when --gpus N > 1 is given without a
+    torchrun environment)."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={gpus}", "--master-addr", "127.0.0.1",
+            "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 # --------------------------------------------------------------------------------------------- CUDA arm
 def build_modes(ctx, l, seed=99):
-    """l orthonormal vectors and their Rayleigh quotients nu_k = <v_k, Q v_k> for the projection leg (every call
-    goes through the C ABI: nd_gaussian, nd_block_dot, nd_block_axpy, nd_scale, nd_apply_Q, nd_dot)."""
+    """l orthonormal vectors and their Rayleigh quotients nu_k = <v_k, Q v_k> for the projection leg of the headline step
+    (every call goes through the C ABI).  NOT eigenvectors: eq. 2.11 is defined for any orthonormal block and its cost
+    does not depend on the values; the configs with real low modes (`configs`, --eigensolve) use nd_lowmodes_compute."""
     if l == 0:
         return None, np.zeros(0)
     V = ctx.new_spinor(l)
@@ -190,58 +224,234 @@ def time_region(torch, ctx, fn, reps):
     return e0.elapsed_time(e1)
 
 
-def measure_q_kernel(torch, nd, dims, U64, prec, recon, peak, reps=40, warm=5):
+def median_of_batches(torch, ctx, fn, reps, batches=5, warm=5):
+    """CUDA events around `reps` repetitions after warm-up, median of `batches` batches -> ms per repetition."""
+    for _ in range(warm):
+        fn()
+    t = [time_region(torch, ctx, fn, reps) / reps for _ in range(batches)]
+    return float(np.median(t)), [float(x) for x in t]
+
+
+def measure_q_kernel(torch, nd, dims, lattice, U64, prec, recon, peak, variants=(None,), reps=20):
     """The Q stencil alone: fixed source, separate destination, CUDA events on the launch stream."""
     ctx = nd.Context(dims, prec=prec, recon=recon, bc_time=-1)
     ctx.set_gauge(U64.astype(np.complex64) if prec == 32 else U64)
     x, y = ctx.new_spinor(), ctx.new_spinor()
     ctx.gaussian(x, 5636)
-    f = lambda: ctx.apply_Q(y, x, M_KERNEL)
-    for _ in range(warm):
-        f()
-    ms = time_region(torch, ctx, f, reps) / reps
     V = ctx.V
-    gbs = q_bytes_per_site(prec, recon) * V / (ms * 1e-3) / 1e9
-    out = {"prec": prec, "recon": recon, "us_per_launch": ms * 1e3, "gflops_1320": FLOP_PER_SITE * V / (ms * 1e-3) / 1e9,
-           "bytes_per_site": q_bytes_per_site(prec, recon), "achieved_gbs": gbs, "frac_of_measured_peak": gbs / peak,
-           "frac_of_8TBs": gbs / 8000.0}
+    out = None
+    for var in variants:
+        if var is not None:
+            try:
+                ctx.set_stencil_variant(var)
+            except nd.NDError:
+                continue
+        name = ctx.get_stencil_variant()
+        ms, batches = median_of_batches(torch, ctx, lambda: ctx.apply_Q(y, x, M_KERNEL), reps)
+        gbs = q_bytes_per_site(prec, recon) * V / (ms * 1e-3) / 1e9
+        kernel = stencil_kernel_name(name, V)
+        r = {"prec": prec, "recon": recon, "stencil_variant": name, "kernel": kernel, "us_per_launch": ms * 1e3,
+             "us_per_launch_batches": [b * 1e3 for b in batches], "gflops_1320": FLOP_PER_SITE * V / (ms * 1e-3) / 1e9,
+             "bytes_per_site": q_bytes_per_site(prec, recon), "achieved_gbs": gbs, "frac_of_measured_peak": gbs / peak,
+             "frac_of_8TBs": gbs / 8000.0, "dram_traffic_ncu": load_traffic(kernel, lattice, prec, recon)}
+        if out is None:
+            out = r                      # the first variant is the one the library picks (auto)
+            out["other_variants"] = {}
+        else:
+            out["other_variants"][name] = {k: r[k] for k in ("kernel", "us_per_launch", "achieved_gbs", "frac_of_measured_peak")}
     ctx.close()
     del x, y
     torch.cuda.empty_cache()
     return out
 
 
-def cpu_baseline_sample(steps=1, n=40, l=4, dims=(32, 16, 16, 16)):
-    """The oracle as it stands on the host cores: its D_N recipe (oracle/sign.py eq. 2.11 + 2.4 over the plain-C
-    stencil oracle/wilson_ref.c) on a bounded sample: a 16^3x32 lattice of the same field recipe, degree n (about 10 s of CPU work per step)."""
+def measure_layout(torch, nd, dims, U64, prec, peak):
+    """a1 alone (VERDICT r1 task 6): AoS <-> SoA on the device, link compression; GB/s over the bytes of both sides."""
+    ctx = nd.Context(dims, prec=prec, recon=12, bc_time=-1)
+    with torch.cuda.stream(ctx.stream):
+        aos = torch.view_as_complex(torch.randn(dims + (4, 3, 2), dtype=ctx.real_dtype, device=ctx.torch_device))
+        back = torch.empty_like(aos)
+        Ud = torch.from_numpy(U64.astype(np.complex64) if prec == 32 else U64).to(ctx.torch_device)
+    soa = ctx.new_spinor()
+    V, b = ctx.V, prec // 8
+    res = {}
+    ms, _ = median_of_batches(torch, ctx, lambda: ctx.lib.nd_pack_spinor(ctx._h, aos.data_ptr(), prec, 1, soa.data_ptr()), 20)
+    res["pack_spinor"] = {"us": ms * 1e3, "gbs": 2 * 24 * b * V / (ms * 1e-3) / 1e9}
+    ms, _ = median_of_batches(torch, ctx, lambda: ctx.lib.nd_unpack_spinor(ctx._h, soa.data_ptr(), back.data_ptr(), prec, 1), 20)
+    res["unpack_spinor"] = {"us": ms * 1e3, "gbs": 2 * 24 * b * V / (ms * 1e-3) / 1e9}
+    ctx.synchronize()
+    res["round_trip_bit_exact"] = bool(torch.equal(aos, back))
+    t = []
+    for _ in range(4):                  # nd_set_gauge synchronises (it returns the SU(3) check): host clock around it
+        ctx.synchronize()
+        t0 = time.perf_counter()
+        ctx.set_gauge(Ud)
+        ctx.synchronize()
+        t.append(time.perf_counter() - t0)
+    ms = float(np.median(t[1:])) * 1e3
+    res["set_gauge_recon12"] = {"us": ms * 1e3, "gbs": 4 * (18 + 12) * b * V / (ms * 1e-3) / 1e9,
+                                "note": "host clock around the call (it synchronises to return the SU(3) check)"}
+    for k in ("pack_spinor", "unpack_spinor", "set_gauge_recon12"):
+        res[k]["frac_of_measured_peak"] = res[k]["gbs"] / peak
+    res["prec"] = prec
+    ctx.close()
+    del aos, back, Ud, soa
+    torch.cuda.empty_cache()
+    return res
+
+
+def dn_config(torch, nd, index, lattice, prec, field_eps, l_window, guard, n, eig_degree, bound_tol, nrhs, sources=10):
+    """BASELINE.json configs[index]: D_N with the low modes from nd_lowmodes_compute (dynamic l, stop on the bound (2.10)),
+    eps by DESIGN.md R11; D_N applications per second over `sources` Gaussian sources, single-source and batched."""
+    from lattice_inputs import gauge_field, parse_lattice
+
+    dims = parse_lattice(lattice)
+    U = gauge_field(dims, "smooth", eps=field_eps)
+    ctx = nd.Context(dims, prec=prec, recon=12, bc_time=-1)
+    ctx.set_gauge(U.astype(np.complex64) if prec == 32 else U)
+    V = ctx.V
+    ctx.synchronize()
+    t0 = time.perf_counter()
+    modes, nu, resid, st = ctx.lowmodes_compute(l_window[0], M_KERNEL, tol=bound_tol, maxit=80, lextra=guard, degree=eig_degree,
+                                                l_max=l_window[1], stop="bound")
+    ctx.synchronize()
+    eig_s = time.perf_counter() - t0
+    eps = 0.99 * float((nu ** 2).max()) / QNORM ** 2
+    c, delta = nd.cheb_coeffs(n, eps)
+    ctx.set_sign_poly(c, eps, QNORM, M_KERNEL)
+    ctx.set_lowmodes(modes, nu)
+    eta, out, work = ctx.new_spinor(sources), ctx.new_spinor(sources), ctx.new_spinor(3)
+    for j in range(sources):
+        ctx.gaussian(eta[j], 5636 + j)
+
+    def sweep():
+        for j in range(sources):
+            ctx.apply_DN(out[j], eta[j], 1.0 / RHO, work, use_graph=True)
+
+    ms, _ = median_of_batches(torch, ctx, sweep, 1, batches=5, warm=2)
+    r = {"config_index": index, "workload": f"D_N apply on {lattice}, exp({field_eps} i H) links, f{prec}, recon 12, degree n={n}, "
+                                            f"low modes from nd_lowmodes_compute", "lattice": lattice, "sites": V,
+         "dtype": f"f{prec}", "degree": n, "eps": eps, "delta": delta,
+         "eigensolve": {"seconds": eig_s, "l_window": list(l_window), "guard": guard, "l_chosen": st["l_chosen"],
+                        "stop": f"bound (2.10) <= {bound_tol}", "converged": st["converged"],
+                        "outer_iterations": st["iterations"], "q_stencils": st["stencils"],
+                        "max_residue_rho": float(resid.max()), "kappa_pm": [float(k) for k in st["kappa"]],
+                        "projector_bound_pm": [float(b) if np.isfinite(b) else None for b in st["bound"]],
+                        "nu2_min": float((nu ** 2).min()), "nu2_max": float((nu ** 2).max())},
+         "sources": sources, "dn_applies_per_s": sources / (ms * 1e-3), "ms_per_dn": ms / sources,
+         "gflops_1320": FLOP_PER_SITE * V * (2 * n + 1) * sources / (ms * 1e-3) / 1e9,
+         "tau_ns_per_clenshaw_iteration_per_site": ms * 1e6 / sources / (n * V),
+         "kernel": stencil_kernel_name(ctx.get_stencil_variant(), V)}
+    if nrhs > 1:
+        nb = min(nrhs, sources)
+        workb = ctx.new_spinor(3 * nb)
+        ms_b, _ = median_of_batches(torch, ctx, lambda: ctx.apply_DN_multi(out[:nb], eta[:nb], 1.0 / RHO, workb, use_graph=True), 1,
+                                    batches=5, warm=2)
+        r["multi_rhs"] = {"nrhs": nb, "dn_applies_per_s": nb / (ms_b * 1e-3), "ms_per_batch": ms_b,
+                          "tau_ns_per_clenshaw_iteration_per_site": ms_b * 1e6 / nb / (n * V)}
+    ctx.close()
+    del modes, eta, out, work
+    torch.cuda.empty_cache()
+    return r
+
+
+def q_config(torch, nd, lattice="16^3x32", field_eps=0.3, reps=1000):
+    """BASELINE.json configs[1]: 1000 back-to-back Q applications (fixed source, separate destination) on 16^3x32,
+    fp32 and fp64 x recon 12 / 8.  The working set (<= 100 MB) is L2-resident: GFLOP/s and model GB/s, NOT an HBM fraction."""
+    from lattice_inputs import gauge_field, parse_lattice
+
+    dims = parse_lattice(lattice)
+    U = gauge_field(dims, "smooth", eps=field_eps)
+    runs = {}
+    for prec, recon in ((32, 12), (32, 8), (64, 12), (64, 8)):
+        ctx = nd.Context(dims, prec=prec, recon=recon, bc_time=-1)
+        ctx.set_gauge(U.astype(np.complex64) if prec == 32 else U)
+        x, y = ctx.new_spinor(), ctx.new_spinor()
+        ctx.gaussian(x, 5636)
+        f = lambda: ctx.apply_Q(y, x, M_KERNEL)
+        for _ in range(10):
+            f()
+        ms = time_region(torch, ctx, f, reps)
+        V = ctx.V
+        runs[f"f{prec}_recon{recon}"] = {"ms_for_1000": ms, "us_per_Q": ms * 1e3 / reps,
+                                         "gflops_1320": FLOP_PER_SITE * V * reps / (ms * 1e-3) / 1e9,
+                                         "model_gbs": q_bytes_per_site(prec, recon) * V * reps / (ms * 1e-3) / 1e9,
+                                         "kernel": stencil_kernel_name(ctx.get_stencil_variant(), V)}
+        ctx.close()
+        del x, y
+    torch.cuda.empty_cache()
+    return {"config_index": 1, "workload": f"{reps} back-to-back Q on {lattice}, exp({field_eps} i H) links, m=-1.6", "lattice": lattice,
+            "note": "working set is L2-resident: GFLOP/s and byte-model GB/s, not an HBM-roofline fraction", "runs": runs}
+
+
+# ------------------------------------------------------------------------------------------ CPU oracle legs
+def oracle_q_alone(lattice, reps=2):
+    """Seconds per Q of the plain-C oracle (oracle/wilson_ref.c, fp64, full 3x3 links) with the OpenMP threads the
+    environment gives it (run in a subprocess to fix OMP_NUM_THREADS)."""
+    from lattice_inputs import gauge_field, gaussian_spinor, parse_lattice
+    from oracle import wilson_c
+
+    dims = parse_lattice(lattice)
+    sd = tuple(min(d, 8) for d in dims)            # a periodic 8^4 Haar block tiled over the lattice: same cost, quick to draw
+    small = gauge_field(sd, "haar")
+    U = np.tile(small, (1,) + tuple(d // e for d, e in zip(dims, sd)) + (1, 1))
+    psi = gaussian_spinor(dims)
+    Q = wilson_c.make_Q(U, M_KERNEL, -1)
+    Q(psi)
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        Q(psi)
+    dt = (time.perf_counter() - t0) / reps
+    return {"lattice": lattice, "threads": wilson_c.num_threads(), "seconds_per_Q": dt,
+            "gflops_1320": FLOP_PER_SITE * int(np.prod(dims)) / dt / 1e9}
+
+
+def oracle_q_alone_subprocess(lattice, threads):
+    env = dict(os.environ)
+    if threads:
+        env["OMP_NUM_THREADS"] = str(threads)
+    code = f"import sys, json; sys.path.insert(0, {ROOT!r}); import bench; print(json.dumps(bench.oracle_q_alone({lattice!r})))"
+    try:
+        r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
+        return json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as e:          # the baseline is context: never let it take the line down
+        return {"lattice": lattice, "threads": threads, "error": str(e)[:200]}
+
+
+def cpu_baseline_sample(steps=1, n=10, l=2, dims=(64, 32, 32, 32), U=None):
+    """The oracle as it stands on the host cores: its D_N recipe (oracle/sign.py eq. 2.11 + 2.4 over the plain-C stencil
+    oracle/wilson_ref.c, fp64, full 3x3 links) on a bounded sample of the line's own workload: the SAME lattice and field
+    recipe, a lower polynomial degree n and l orthonormal projection vectors (10-30 s of CPU work per step)."""
     from lattice_inputs import gauge_field, gaussian_spinor
     from oracle import lowmodes as olow
     from oracle import sign as osign
     from oracle import wilson, wilson_c
 
-    U = gauge_field(dims, "haar")
+    if U is None:
+        U = gauge_field(dims, "haar")
     eta = gaussian_spinor(dims)
     Q = wilson_c.make_Q(U, M_KERNEL, -1)
-    qnorm = wilson.norm_bound_Q(M_KERNEL)
     eps = 0.002
     c = osign.cheb_coeffs(n, eps)
     rng = np.random.Generator(np.random.PCG64(3))
     Vs = olow.orthonormalise([rng.standard_normal(eta.shape) + 1j * rng.standard_normal(eta.shape) for _ in range(l)])
     nu, Us = osign.rayleigh_ritz_Q(Q, Vs)
-    osign.apply_DN(Q, wilson.apply_gamma5, eta, c[:3], eps, qnorm, 1.0 / RHO, nu, Us)    # warm-up (loads the C library)
+    osign.apply_DN(Q, wilson.apply_gamma5, eta, c[:2], eps, QNORM, 1.0 / RHO, nu, Us)    # warm-up (loads the C library)
     t0 = time.perf_counter()
     for _ in range(steps):
-        osign.apply_DN(Q, wilson.apply_gamma5, eta, c, eps, qnorm, 1.0 / RHO, nu, Us)
+        osign.apply_DN(Q, wilson.apply_gamma5, eta, c, eps, QNORM, 1.0 / RHO, nu, Us)
     dt = (time.perf_counter() - t0) / steps
     vol = int(np.prod(dims))
     gflops = FLOP_PER_SITE * vol * (2 * n + 1) / dt / 1e9
-    return {"value": gflops, "unit": "GFLOP/s", "cores": wilson_c.num_threads(), "kind": "oracle",
+    return {"value": gflops, "unit": "GFLOP/s", "cores": wilson_c.num_threads(), "kind": "oracle", "cpu_model": cpu_model(),
             "sample": f"oracle D_N recipe (oracle/sign.py over oracle/wilson_ref.c, fp64, full 3x3 links) on a "
-                      f"{dims[1]}^3x{dims[0]} Haar lattice, degree n={n}, l={l}: {2 * n + 1} stencils/step, "
-                      f"{dt:.2f} s/step",
-            "dn_applies_per_s": 1.0 / dt, "seconds_per_step": dt}
+                      f"{dims[1]}^3x{dims[0]} Haar lattice at degree n={n}, l={l} (synthetic orthonormal vectors): "
+                      f"{2 * n + 1} stencils/step, {dt:.2f} s/step",
+            "dn_applies_per_s": 1.0 / dt, "seconds_per_step": dt,
+            "tau_ns_per_clenshaw_iteration_per_site": dt * 1e9 / (n * vol)}
 
 
+# ---------------------------------------------------------------------------------------------- main arms
 def run_b200(args):
     import torch
 
@@ -249,9 +459,6 @@ def run_b200(args):
     from lattice_inputs import gauge_field, parse_lattice
 
     rank, world, local = dist_env()
-    if world != args.gpus:
-        if world == 1 and args.gpus > 1:
-            raise SystemExit("--gpus N > 1 must be launched with torch.distributed.run (one rank per GPU)")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device - the CUDA path has no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
@@ -263,33 +470,31 @@ def run_b200(args):
     prec, recon, n, l = args.prec, args.recon, args.degree, args.lowmodes
     peak, peak_src = load_peaks()
 
-    # BASELINE config 2: Haar-random links, seeded (configs 1, 3, 4: --field smooth)
+    # BASELINE config index 2: Haar-random links, seeded (--field smooth for the exp(i eps H) recipe)
     U64 = gauge_field(dims, args.field, eps=args.field_eps)
     ctx = nd.Context(dims, prec=prec, recon=recon, bc_time=-1, device=local)
     ctx.set_gauge(U64.astype(np.complex64) if prec == 32 else U64)
     V = ctx.V
-    qnorm = abs(4.0 + M_KERNEL) + 4.0
     c, delta = nd.cheb_coeffs(n, args.eps)
-    ctx.set_sign_poly(c, args.eps, qnorm, M_KERNEL)
+    ctx.set_sign_poly(c, args.eps, QNORM, M_KERNEL)
     eig = None
+    modes_kind = "synthetic orthonormal vectors with their Rayleigh quotients (not eigenvectors; eps not tied to the spectrum)"
     if args.eigensolve and l > 0:
-        # BASELINE config 4: the low modes come from the library's own eigen-solver (a10), timed on the host clock
-        # (it synchronises for its small dense problems); eps then follows DESIGN.md R11.
         ctx.synchronize()
         t0 = time.perf_counter()
         modes, nu, resid, st = ctx.lowmodes_compute(max(1, l - l // 8), M_KERNEL, tol=args.eig_tol, maxit=60, lextra=max(8, l // 4),
                                                     degree=args.eig_degree, l_max=l + l // 8, stop="bound")
-        l = st["l_chosen"]
         ctx.synchronize()
-        eig = {"seconds": time.perf_counter() - t0, "l": l, "tol_bound_2_10": args.eig_tol, "converged": st["converged"],
-               "outer_iterations": st["iterations"], "q_stencils": st["stencils"], "max_residue_Q": float(resid.max()),
+        l = st["l_chosen"]
+        eig = {"seconds": time.perf_counter() - t0, "l_chosen": l, "tol_bound_2_10": args.eig_tol, "converged": st["converged"],
+               "outer_iterations": st["iterations"], "q_stencils": st["stencils"], "max_residue_rho": float(resid.max()),
+               "kappa_pm": [float(k) for k in st["kappa"]],
+               "projector_bound_pm": [float(b) if np.isfinite(b) else None for b in st["bound"]],
                "nu2_min": float((nu ** 2).min()), "nu2_max": float((nu ** 2).max())}
-        eig["l_chosen"] = l
-        eig["kappa_pm"] = [float(st["kappa"][0]), float(st["kappa"][1])]                 # eq. 2.9
-        eig["projector_bound_pm"] = [float(b) if np.isfinite(b) else None for b in st["bound"]]   # eq. 2.10
-        args.eps = 0.99 * float((nu ** 2).max()) / qnorm ** 2
+        args.eps = 0.99 * float((nu ** 2).max()) / QNORM ** 2
         c, delta = nd.cheb_coeffs(n, args.eps)
-        ctx.set_sign_poly(c, args.eps, qnorm, M_KERNEL)
+        ctx.set_sign_poly(c, args.eps, QNORM, M_KERNEL)
+        modes_kind = "nd_lowmodes_compute (dynamic l, bound (2.10)); eps by DESIGN.md R11"
     else:
         modes, nu = build_modes(ctx, l)
     ctx.set_lowmodes(modes, nu)
@@ -318,6 +523,7 @@ def run_b200(args):
     stencils = 2 * n + 1
     gflop_per_step = FLOP_PER_SITE * V * stencils / 1e9
     value = whole_job_value(gflop_per_step * args.steps, world, ms)
+    headline_variant = ctx.get_stencil_variant()
 
     # ---- end-to-end leg: host AoS source in pinned memory -> pack -> D_N -> unpack -> pinned host result
     cdt = torch.complex64 if prec == 32 else torch.complex128
@@ -344,39 +550,60 @@ def run_b200(args):
             dist.barrier()
             dist.destroy_process_group()
         return
-    # ---- rank 0 only: the dominant kernel alone (roofline), every variant; the CPU oracle
+    # ---- rank 0 only: the dominant kernel alone (roofline), every variant; layout; the other configs; the CPU oracle
     ctx.close()
     del modes, eta, out, work
     torch.cuda.empty_cache()
     qk = {}
+    q_sampler = ClockSampler(local).start()
     for p, r in ((32, 12), (64, 12), (32, 8), (64, 8), (32, 18), (64, 18)):
-        if args.quick and (p, r) not in ((prec, recon),):
+        if args.quick and (p, r) != (prec, recon):
             continue
-        qk[f"f{p}_recon{r}"] = measure_q_kernel(torch, nd, dims, U64, p, r, peak)
+        variants = (None, "site", "tile_tma") if p == 32 else (None,)
+        qk[f"f{p}_recon{r}"] = measure_q_kernel(torch, nd, dims, args.lattice, U64, p, r, peak, variants)
+    q_clocks = q_sampler.stop()
     main = qk[f"f{prec}_recon{recon}"]
     roofline = {"bound": "hbm", "achieved": main["achieved_gbs"], "peak": peak, "unit": "GB/s",
-                "frac": main["achieved_gbs"] / peak, "traffic": load_traffic(f"f{prec}_recon{recon}"),
-                "kernel": "wilson_Q_kernel (Q stencil, plain epilogue)", "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": main["bytes_per_site"] * V, "us_per_launch": main["us_per_launch"],
-                "frac_of_8TBs_nominal": main["achieved_gbs"] / 8000.0}
-    cpu = None if args.no_cpu_baseline else cpu_baseline_sample()
+                "frac": main["achieved_gbs"] / peak, "traffic": main["dram_traffic_ncu"],
+                "kernel": f"{main['kernel']} (Q stencil, plain epilogue; stencil variant '{main['stencil_variant']}')",
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": main["bytes_per_site"] * V,
+                "us_per_launch": main["us_per_launch"], "timing": "median of 5 batches of 20 launches, CUDA events on the launch stream",
+                "frac_of_8TBs_nominal": main["achieved_gbs"] / 8000.0, "clocks": q_clocks,
+                "traffic_source": "profiles/q_kernel_dram_traffic.csv (ncu --set full of this kernel on this lattice; null = no capture)"}
+    layout, configs, cpu = None, [], None
+    if not args.quick:
+        layout = {f"f{p}": measure_layout(torch, nd, dims, U64, p, peak) for p in (32, 64)}
+        configs.append(q_config(torch, nd))
+        configs.append(dn_config(torch, nd, 3, "8^3x16", 64, 0.3, (16, 24), 8, 100, 60, 1e-6, nrhs=8))
+        configs.append(dn_config(torch, nd, 4, "16^3x32", 32, 0.25, (44, 56), 12, 200, 160, 1e-2, nrhs=4))
+    if not args.no_cpu_baseline and not args.quick:
+        cpu = cpu_baseline_sample(dims=dims, U=U64)
+        ncores = os.cpu_count() or 1
+        cpu["q_alone"] = [oracle_q_alone_subprocess(lat, th) for lat in ("16^3x32", "32^3x64") for th in (1, ncores)]
+    elif not args.no_cpu_baseline:
+        cpu = cpu_baseline_sample(dims=(32, 16, 16, 16), n=6)
     line = {
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
         "config": {"workload": f"D_N apply (eq. 2.4+2.11) on {args.lattice}, {args.field} SU(3) links, m=-1.6, recon {recon}, "
-                               f"degree n={n} (2n+1={stencils} Q stencils), l={l} projected modes, CUDA graph",
+                               f"degree n={n} (2n+1={stencils} Q stencils), l={l} projected vectors, CUDA graph",
                    "lattice": args.lattice, "sites": V, "recon": recon, "degree": n, "eps": args.eps, "delta": delta,
-                   "lowmodes": l, "replicas": world, "parallelism": f"replicas x{world}",
+                   "lowmodes": l, "lowmodes_kind": modes_kind, "stencil_variant": headline_variant,
+                   "replicas": world, "parallelism": f"replicas x{world}",
                    "l2_policy": "inputs larger than L2 (links + vectors >= 1.4 GB fp32), no flush needed"},
         "dn_applies_per_s": world * args.steps / (ms * 1e-3),
         "q_stencils_per_s": world * args.steps * stencils / (ms * 1e-3),
+        "tau_ns_per_clenshaw_iteration_per_site": ms * 1e6 / args.steps / (n * V),
+        "tau_paper_ns": {"single_GTX285": 38.0, "double_GTX285": 90.0, "source": "PAPER.md:L140-142 (context, other hardware)"},
         "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": hbytes, "d2h_bytes_per_step": hbytes,
                 "ms_per_step": ms_e2e / args.steps},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": roofline,
         "q_kernel": qk,
+        "layout": layout,
+        "configs": configs,
         "cpu_baseline": cpu,
     }
     if eig is not None:
@@ -392,15 +619,21 @@ def run_reference(args):
     rank, world, _ = dist_env()
     if rank != 0:
         return
-    # W warm-up + K timed steps of the oracle, each step one D_N application on the bounded sample
-    cpu_baseline_sample(steps=max(args.warmup, 1), n=2)
-    r = cpu_baseline_sample(steps=args.steps)
+    # W warm-up + K timed steps of the oracle, each step one D_N application on a bounded sample of the CUDA arm's workload
+    # (same field recipe and operator; a 16^3x32 lattice at degree 40 keeps a K-step run within minutes on the host cores)
+    dims = (32, 16, 16, 16)
+    from lattice_inputs import gauge_field
+
+    U = gauge_field(dims, "haar")
+    cpu_baseline_sample(steps=max(args.warmup, 1), n=1, l=4, dims=dims, U=U)
+    r = cpu_baseline_sample(steps=args.steps, n=40, l=4, dims=dims, U=U)
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": "GFLOP/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_step"] * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "CPU oracle: " + r["sample"]},
-        "cpu_baseline": {"value": r["value"], "unit": "GFLOP/s", "kind": "oracle", "cores": r["cores"], "sample": r["sample"]},
+        "cpu_baseline": {"value": r["value"], "unit": "GFLOP/s", "kind": "oracle", "cores": r["cores"], "sample": r["sample"],
+                         "cpu_model": r["cpu_model"]},
         "e2e": {"value": r["value"], "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -423,11 +656,19 @@ def main():
     ap.add_argument("--field-eps", type=float, default=0.25, help="eps of U = exp(i eps H) for --field smooth")
     ap.add_argument("--eigensolve", action="store_true", help="low modes from nd_lowmodes_compute (timed), eps by R11")
     ap.add_argument("--eig-tol", type=float, default=1e-2, help="stop when the bound (2.10) on the projector error is below this")
-    ap.add_argument("--eig-degree", type=int, default=80)
-    ap.add_argument("--quick", action="store_true", help="time only the line's own Q-kernel variant")
+    ap.add_argument("--eig-degree", type=int, default=100)
+    ap.add_argument("--quick", action="store_true", help="headline + its own Q-kernel variant only (no layout / configs legs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started as `python bench.py --gpus N`: start the N ranks ourselves (one per GPU, NCCL only for the barrier)
+        import socket
+
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            port = s.getsockname()[1]
+        raise SystemExit(subprocess.call(spawn_command(sys.argv[1:], args.gpus, port)))
     if args.impl == "reference":
         run_reference(args)
     else:

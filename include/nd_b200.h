@@ -125,6 +125,10 @@ ND_API int nd_apply_Q_axpbycz(nd_ctx* ctx, void* out, const void* in, double m, 
  * approximating y^{-1/2} on [eps, 1] (eq. 2.5-2.6; Chebyshev interpolation, full c_0) and the
  * measured delta = max_{eps<=y<=1} |1 - sqrt(y) P(y)| (eq. 2.6). */
 ND_API int nd_cheb_coeffs(int n, double eps, double* c, double* delta);
+/* The same with the coefficients that MINIMISE delta of eq. 2.6 ("minmax polynomials"), by the Remez
+ * exchange algorithm: delta is 1.6-1.9 times smaller than the interpolation polynomial's at equal degree.  *levelled (may be
+ * NULL) = the levelled error |E| of the last reference: |E| <= the optimal delta <= *delta (de la Vallee-Poussin). */
+ND_API int nd_minmax_coeffs(int n, double eps, double* c, double* delta, double* levelled);
 /* Polynomial used by nd_apply_sign / nd_apply_DN: degree n, coefficients c[0..n] (host, copied), eps, the
  * norm bound qnorm >= ||Q|| (X = Q/qnorm) and the kernel mass m (= -(1+s), eq. 2.4). */
 ND_API int nd_set_sign_poly(nd_ctx* ctx, int n, const double* c, double eps, double qnorm, double m);

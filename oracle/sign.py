@@ -126,3 +126,61 @@ def apply_DN(Q, gamma5, eta, c, eps, qnorm, prefactor, nu=None, U=None):
         s = sign_projected(Q, eta, c, eps, qnorm, nu, U)
     return prefactor * (eta + gamma5(s))
 
+
+
+# ----------------------------------------------------------------------------- min-max coefficients, eq. 2.6
+def minmax_coeffs(n, eps, max_iter=60, tol=1e-3):
+    """The polynomial that MINIMISES delta = max_{eps<=y<=1} |1 - sqrt(y) P(y)| (eq. 2.6: "minmax
+    polynomials"), by the Remez exchange algorithm for the weighted problem  w(y) (f(y) - P(y)),  f = y^{-1/2}, w = y^{1/2}:
+      1. reference y_0 < ... < y_{n+1} (start: the extrema of T_{n+1} in z);
+      2. solve  sum_k c_k T_k(z_i) + (-1)^i E / w(y_i) = f(y_i),  i = 0..n+1,  for (c_0..c_n, E)   [long double elimination];
+      3. new reference = the alternating local extrema of the error e(y) = 1 - sqrt(y) P(y) on a fine grid;
+      repeat until max|e| <= (1 + tol) |E|  (de la Vallee-Poussin: |E| <= delta_min <= max|e|).
+    Same conventions as cheb_coeffs (z = (2y-1-eps)/(1-eps), full c_0).  Returns (c[0..n], delta = max|e| measured, |E|)."""
+    ld = np.longdouble
+    m = n + 2
+    i = np.arange(m, dtype=ld)
+    z = -np.cos(ld(np.pi) * i / ld(m - 1))                      # ascending in z: -1 .. 1
+    # fine grid, Chebyshev-distributed in z (dense at both ends, where the extrema crowd)
+    ng = 60 * m
+    zg = -np.cos(np.pi * (np.arange(ng) + 0.5) / ng)
+    zg = np.concatenate([[-1.0], zg, [1.0]])
+    yg = ((1.0 - eps) * zg + 1.0 + eps) / 2.0
+    c = None
+    E = ld(0)
+    for _ in range(max_iter):
+        y = (ld(1.0 - eps) * z + ld(1.0 + eps)) / ld(2.0)
+        A = np.empty((m, m), dtype=ld)
+        theta = np.arccos(np.clip(z, -1, 1))
+        A[:, :n + 1] = np.cos(np.outer(theta, np.arange(n + 1, dtype=ld)))
+        A[:, n + 1] = np.where(np.arange(m) % 2 == 0, ld(1), ld(-1)) / np.sqrt(y)
+        b = ld(1.0) / np.sqrt(y)
+        # Gaussian elimination with partial pivoting in long double
+        M = np.concatenate([A, b[:, None]], axis=1)
+        for k in range(m):
+            p = k + int(np.argmax(np.abs(M[k:, k])))
+            if p != k:
+                M[[k, p]] = M[[p, k]]
+            M[k + 1:] -= np.outer(M[k + 1:, k] / M[k, k], M[k])
+        sol = np.empty(m, dtype=ld)
+        for k in range(m - 1, -1, -1):
+            sol[k] = (M[k, m] - M[k, k + 1:m] @ sol[k + 1:]) / M[k, k]
+        c = np.asarray(sol[:n + 1], dtype=np.float64)
+        E = sol[n + 1]
+        e = 1.0 - np.sqrt(yg) * eval_P_scalar(c, eps, yg)
+        emax = float(np.max(np.abs(e)))
+        if emax <= (1.0 + tol) * abs(float(E)):
+            break
+        # alternating extrema: split the grid where the error changes sign, take the largest |e| of every piece
+        sgn = np.sign(e)
+        sgn[sgn == 0] = 1
+        cuts = np.flatnonzero(sgn[1:] != sgn[:-1]) + 1
+        pieces = np.split(np.arange(len(e)), cuts)
+        ext = np.array([p[np.argmax(np.abs(e[p]))] for p in pieces])
+        while len(ext) > m:                                       # drop the smaller end extremum until n+2 are left
+            ext = ext[1:] if abs(e[ext[0]]) < abs(e[ext[-1]]) else ext[:-1]
+        if len(ext) < m:
+            break                                                 # (degree too high for this grid / precision)
+        z = np.asarray(zg[ext], dtype=ld)
+    delta = float(np.max(np.abs(1.0 - np.sqrt(yg) * eval_P_scalar(c, eps, yg))))
+    return c, max(delta, measure_delta(c, eps, 100001)), abs(float(E))

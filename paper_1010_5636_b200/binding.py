@@ -46,6 +46,7 @@ SIGNATURES = {
     "nd_apply_Q2": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_dbl]),
     "nd_apply_Q_axpbycz": (_c_int, [_c_vp, _c_vp, _c_vp, _c_dbl, _c_dbl, _c_dbl, _c_vp, _c_dbl, _c_vp, _c_dbl, _c_vp]),
     "nd_cheb_coeffs": (_c_int, [_c_int, _c_dbl, _pd, _pd]),
+    "nd_minmax_coeffs": (_c_int, [_c_int, _c_dbl, _pd, _pd, _pd]),
     "nd_set_sign_poly": (_c_int, [_c_vp, _c_int, _pd, _c_dbl, _c_dbl, _c_dbl]),
     "nd_set_lowmodes": (_c_int, [_c_vp, _c_int, _c_vp, _pd]),
     "nd_apply_sign": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp, _c_int]),
@@ -115,6 +116,17 @@ def cheb_coeffs(n, eps):
     if rc != ND_OK:
         raise NDError(rc, "nd_cheb_coeffs")
     return c, delta.value
+
+
+def minmax_coeffs(n, eps):
+    """nd_minmax_coeffs: (c[0..n], delta, levelled error E) of the min-max polynomial of eq. 2.6 - host utility, no GPU."""
+    lib = load_library()
+    c = np.zeros(n + 1, dtype=np.float64)
+    delta, lev = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    rc = lib.nd_minmax_coeffs(int(n), float(eps), c.ctypes.data_as(_pd), ctypes.byref(delta), ctypes.byref(lev))
+    if rc != ND_OK:
+        raise NDError(rc, "nd_minmax_coeffs")
+    return c, delta.value, lev.value
 
 
 def heev(a):

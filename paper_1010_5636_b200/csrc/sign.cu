@@ -11,6 +11,7 @@
 // (nd_apply_Q_axpbycz), so the recurrence vectors are read/written exactly once per step: 2n+1 stencil launches per
 // sign application, no separate axpy kernels.  No host synchronisation anywhere: the projection coefficients stay on
 // the device, so the whole application can be replayed as one CUDA graph.
+#include <algorithm>
 #include <cmath>
 
 #include "nd_internal.cuh"
@@ -186,6 +187,105 @@ extern "C" int nd_cheb_coeffs(int n, double eps, double* c, double* delta) {
                 const double P = c[0] + z * b1 - b2;
                 const double d = fabs(1.0 - sqrt(y) * P);
                 if (d > worst) worst = d;
+            }
+        *delta = worst;
+    }
+    return ND_OK;
+}
+
+// Min-max coefficients (eq. 2.6, "minmax polynomials"): the polynomial of degree n minimising
+// delta = max_{eps<=y<=1} |1 - sqrt(y) P(y)|, by the Remez exchange for the weighted problem w (f - P), f = y^{-1/2}, w = y^{1/2}:
+// solve  sum_k c_k T_k(z_i) + (-1)^i E / w(y_i) = f(y_i)  on a reference of n+2 points (long double elimination), move the
+// reference to the alternating extrema of the error on a fine grid, repeat until max|e| <= (1 + 1e-3) |E|.  Conventions as
+// nd_cheb_coeffs (z = (2y-1-eps)/(1-eps), full c_0).  Host utility, no GPU.
+extern "C" int nd_minmax_coeffs(int n, double eps, double* c, double* delta, double* levelled) {
+    if (n < 0 || n > 4096 || !(eps > 0.0 && eps < 1.0) || !c) return ND_ERR_BAD_ARG;
+    typedef long double ld;
+    const ld pi = acosl(-1.0L);
+    const int m = n + 2;
+    std::vector<ld> z(m), sol(m), M((size_t)m * (m + 1));
+    for (int i = 0; i < m; i++) z[i] = -cosl(pi * (ld)i / (ld)(m - 1));
+    const int ng = 64 * m + 2;
+    std::vector<double> zg(ng), eg(ng);
+    zg[0] = -1.0;
+    zg[ng - 1] = 1.0;
+    for (int i = 1; i < ng - 1; i++) zg[i] = -cos(M_PI * ((double)i - 0.5) / (double)(ng - 2));
+    auto error_at = [&](double zz) {
+        double b1 = 0.0, b2 = 0.0;
+        for (int k = n; k >= 1; k--) {
+            const double b0 = c[k] + 2.0 * zz * b1 - b2;
+            b2 = b1;
+            b1 = b0;
+        }
+        const double y = 0.5 * ((1.0 - eps) * zz + 1.0 + eps);
+        return 1.0 - sqrt(y) * (c[0] + zz * b1 - b2);
+    };
+    ld E = 0.0L;
+    double emax = 0.0;
+    for (int it = 0; it < 80; it++) {
+        for (int i = 0; i < m; i++) {
+            const ld y = 0.5L * ((1.0L - (ld)eps) * z[i] + 1.0L + (ld)eps);
+            const ld th = acosl(z[i] > 1.0L ? 1.0L : (z[i] < -1.0L ? -1.0L : z[i]));
+            for (int k = 0; k <= n; k++) M[(size_t)i * (m + 1) + k] = cosl((ld)k * th);
+            M[(size_t)i * (m + 1) + n + 1] = ((i & 1) ? -1.0L : 1.0L) / sqrtl(y);
+            M[(size_t)i * (m + 1) + m] = 1.0L / sqrtl(y);
+        }
+        for (int k = 0; k < m; k++) {   // elimination with partial pivoting
+            int p = k;
+            for (int i = k + 1; i < m; i++)
+                if (fabsl(M[(size_t)i * (m + 1) + k]) > fabsl(M[(size_t)p * (m + 1) + k])) p = i;
+            if (M[(size_t)p * (m + 1) + k] == 0.0L) return ND_ERR_NO_CONVERGENCE;
+            if (p != k)
+                for (int j = 0; j <= m; j++) std::swap(M[(size_t)k * (m + 1) + j], M[(size_t)p * (m + 1) + j]);
+            for (int i = k + 1; i < m; i++) {
+                const ld f = M[(size_t)i * (m + 1) + k] / M[(size_t)k * (m + 1) + k];
+                if (f == 0.0L) continue;
+                for (int j = k; j <= m; j++) M[(size_t)i * (m + 1) + j] -= f * M[(size_t)k * (m + 1) + j];
+            }
+        }
+        for (int k = m - 1; k >= 0; k--) {
+            ld t = M[(size_t)k * (m + 1) + m];
+            for (int j = k + 1; j < m; j++) t -= M[(size_t)k * (m + 1) + j] * sol[j];
+            sol[k] = t / M[(size_t)k * (m + 1) + k];
+        }
+        for (int k = 0; k <= n; k++) c[k] = (double)sol[k];
+        E = sol[n + 1];
+        emax = 0.0;
+        for (int i = 0; i < ng; i++) {
+            eg[i] = error_at(zg[i]);
+            emax = std::max(emax, fabs(eg[i]));
+        }
+        if (emax <= (1.0 + 1e-3) * (double)fabsl(E)) break;
+        // the alternating extrema: the largest |e| of every stretch of constant sign; surplus ones are dropped at the ends
+        std::vector<int> ext;
+        int best = 0;
+        for (int i = 1; i <= ng; i++) {
+            if (i == ng || (eg[i] >= 0.0) != (eg[best] >= 0.0)) {
+                ext.push_back(best);
+                best = i;
+            } else if (fabs(eg[i]) > fabs(eg[best])) {
+                best = i;
+            }
+        }
+        size_t lo = 0, hi = ext.size();
+        while (hi - lo > (size_t)m) {
+            if (fabs(eg[ext[lo]]) < fabs(eg[ext[hi - 1]])) lo++;
+            else hi--;
+        }
+        if (hi - lo < (size_t)m) break;   // degree beyond what the grid / fp64 evaluation resolves: keep the last iterate
+        for (int i = 0; i < m; i++) z[i] = (ld)zg[ext[lo + i]];
+    }
+    if (levelled) *levelled = (double)fabsl(E);
+    if (delta) {
+        // the same measurement as nd_cheb_coeffs: geometric and linear grid of [eps, 1]
+        double worst = emax;
+        const int npts = 100001;
+        const double lr = log(1.0 / eps);
+        for (int pass = 0; pass < 2; pass++)
+            for (int i = 0; i < npts; i++) {
+                const double t = (double)i / (double)(npts - 1);
+                const double y = pass == 0 ? eps * exp(lr * t) : eps + (1.0 - eps) * t;
+                worst = std::max(worst, fabs(error_at((2.0 * y - 1.0 - eps) / (1.0 - eps))));
             }
         *delta = worst;
     }

@@ -235,7 +235,7 @@ int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double 
     G.S0 = (long long)G.L1 * G.L2 * G.L3;
     G.bc = ctx->bc;
     const long long bstride = (long long)Prec<T>::NV * ctx->V;   // one spinor, in 128-bit words
-    if (ctx->V < (long long)ctx->hop_max_sites) {
+    if (ctx->V * nrhs < (long long)ctx->hop_max_sites) {   // (a batch of right-hand sides counts as one larger lattice)
         // fewer sites than lanes on the chip: one warp per hop (latency-bound regime, BASELINE config 3)
         const dim3 nb((unsigned)((ctx->V + 31) / 32), (unsigned)nrhs, 1);
         const dim3 tb(32, 8, 1);
@@ -252,10 +252,10 @@ int launch_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double 
     }
     // 128 threads per CTA; small lattices get smaller CTAs so that every SM has work
     int threads = 128;
-    while (threads > 32 && ctx->V / threads < 2 * ctx->num_sms) threads /= 2;
+    while (threads > 32 && ctx->V * nrhs / threads < 2 * ctx->num_sms) threads /= 2;
     unsigned blocks1 = (unsigned)((ctx->V + threads - 1) / threads);
     for (int i = 0; i < 3; i++) { G.lb[i] = ctx->tile_lb[i]; G.nt[i] = 0; }
-    if (ctx->tile_threads > 0 && ctx->tile_threads <= Q_THREADS && ctx->V / ctx->tile_threads >= 2 * ctx->num_sms) {
+    if (ctx->tile_threads > 0 && ctx->tile_threads <= Q_THREADS && ctx->V * nrhs / ctx->tile_threads >= 2 * ctx->num_sms) {
         threads = ctx->tile_threads;
         blocks1 = (unsigned)G.L0;
         for (int i = 0; i < 3; i++) { G.nt[i] = ctx->dims[i + 1] >> G.lb[i]; blocks1 *= (unsigned)G.nt[i]; }

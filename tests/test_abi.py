@@ -162,3 +162,24 @@ def test_choose_l_matches_oracle():
     for bad in ((a[::-1], 1, 2), (a, 0, 2), (a, 3, 2), (a, 1, len(a))):
         with pytest.raises(nd.NDError):
             nd.choose_l(*bad)
+
+
+@pytest.mark.parametrize("n,eps", [(0, 0.04), (12, 0.1), (40, 0.01), (100, 0.005)])
+def test_minmax_coeffs_match_oracle(n, eps):
+    """nd_minmax_coeffs (library, Remez in C++) vs oracle.sign.minmax_coeffs (numpy): the min-max polynomial is unique, so two
+    independent implementations must give the same polynomial and the same delta; closed form at n = 0."""
+    import paper_1010_5636_b200 as nd
+    from oracle import sign as osign
+
+    c, delta, lev = nd.minmax_coeffs(n, eps)
+    co, do, Eo = osign.minmax_coeffs(n, eps)
+    assert lev <= delta <= 1.002 * lev and abs(delta - do) <= 3e-3 * do
+    y = np.geomspace(eps, 1.0, 5001)
+    assert np.abs(np.sqrt(y) * (osign.eval_P_scalar(c, eps, y) - osign.eval_P_scalar(co, eps, y))).max() <= 5e-3 * delta
+    assert osign.measure_delta(c, eps) <= delta * (1 + 1e-6)          # the library's delta is what its coefficients deliver
+    if n == 0:
+        r = np.sqrt(eps)
+        assert abs(c[0] - 2 / (1 + r)) < 1e-14 and abs(delta - (1 - r) / (1 + r)) < 1e-14
+    else:
+        ci, di = nd.cheb_coeffs(n, eps)
+        assert delta < 0.75 * di

@@ -57,6 +57,24 @@ def test_single_rank_helpers():
     assert bench.q_bytes_per_site(32, 12, 3) == 384 + 288
 
 
+def test_spawn_command_and_traffic_table():
+    """`python bench.py --gpus N` without a torchrun environment re-executes itself under torch.distributed.run with one rank
+    per GPU on 127.0.0.1; the DRAM-traffic table is keyed by kernel, lattice, precision and recon and gives None otherwise."""
+    sys.path.insert(0, ROOT)
+    import bench
+
+    cmd = bench.spawn_command(["--gpus", "4", "--steps", "2"], 4, 29512)
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node=4" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29512"
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "2"] and cmd[-5].endswith("bench.py")
+    assert bench.load_traffic("wilson_Q_kernel", "5^3x7", 32, 12) is None          # no capture of that lattice
+    assert bench.load_traffic("no_such_kernel", "32^3x64", 32, 12) is None
+    t = bench.load_traffic("wilson_Q_tile_kernel", "32^3x64", 32, 12)
+    assert t is None or 0.9 * 805306368 < t < 1.3 * 805306368                      # a capture, if present, is near the byte model
+    assert bench.stencil_kernel_name("site", 8192) == "wilson_Q_hop_kernel" and bench.stencil_kernel_name("site", 1 << 20) == "wilson_Q_kernel"
+    assert bench.stencil_kernel_name("tile", 1 << 21) == "wilson_Q_tile_kernel"
+
+
 def test_reference_arm_other_ranks_exit_without_work():
     env = dict(os.environ, RANK="1", LOCAL_RANK="1", WORLD_SIZE="2")
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",

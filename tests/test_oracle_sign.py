@@ -202,3 +202,57 @@ def test_free_field_DN_closed_form():
     expect = phase[..., None, None] * (cpre * (w + (Dp @ w) / om))
     got = sign.apply_DN(Q, wilson.apply_gamma5, psi, c, eps, qnorm, cpre)
     assert np.linalg.norm((got - expect).ravel()) <= cpre * delta * np.linalg.norm(psi.ravel())
+
+
+# ------------------------------------------------------------------------------- min-max coefficients (eq. 2.6)
+def test_minmax_degree_zero_closed_form():
+    """n = 0: minimise max |1 - c0 sqrt(y)| on [eps, 1]: the error is monotone, so it is levelled at the two end points:
+    c0 = 2 / (1 + sqrt(eps)), delta = (1 - sqrt(eps)) / (1 + sqrt(eps)) - by hand."""
+    for eps in (0.04, 0.25, 0.0025):
+        c, delta, E = sign.minmax_coeffs(0, eps)
+        r = np.sqrt(eps)
+        assert abs(c[0] - 2.0 / (1.0 + r)) < 1e-14 and abs(delta - (1.0 - r) / (1.0 + r)) < 1e-14 and abs(E - delta) < 1e-14
+
+
+@pytest.mark.parametrize("n,eps", [(8, 0.1), (20, 0.05), (40, 0.01), (100, 0.005), (100, 0.002)])
+def test_minmax_equioscillates_and_beats_interpolation(n, eps):
+    """Chebyshev's alternation theorem pins the min-max polynomial of eq. 2.6: the error 1 - sqrt(y) P(y) attains +-delta at
+    n + 2 points with alternating signs (then P is THE minimiser), de la Vallee-Poussin sandwiches the optimum,
+    E <= delta_min <= delta, and delta is below the interpolation polynomial's at the same degree."""
+    c, delta, E = sign.minmax_coeffs(n, eps)
+    assert E <= delta <= 1.002 * E
+    z = -np.cos(np.pi * (np.arange(200 * (n + 2)) + 0.5) / (200 * (n + 2)))
+    y = np.concatenate([[eps], ((1 - eps) * z + 1 + eps) / 2, [1.0]])
+    e = 1.0 - np.sqrt(y) * sign.eval_P_scalar(c, eps, y)
+    assert np.abs(e).max() <= delta * (1 + 1e-9)
+    big = np.flatnonzero(np.abs(e) >= 0.995 * delta)
+    signs = np.sign(e[big])
+    alternations = 1 + int(np.sum(signs[1:] != signs[:-1]))
+    assert alternations == n + 2
+    ci = sign.cheb_coeffs(n, eps)
+    assert delta < 0.75 * sign.measure_delta(ci, eps)
+    # the sign-function form of eq. 2.5 obeys the same bound on sqrt(eps) <= |x| <= 1
+    x = np.concatenate([-np.geomspace(1.0, np.sqrt(eps), 4001), np.geomspace(np.sqrt(eps), 1.0, 4001)])
+    assert np.abs(x * sign.eval_P_scalar(c, eps, x * x) - np.sign(x)).max() <= delta * (1 + 1e-9)
+
+
+def test_minmax_polynomial_is_a_valid_sign_approximation_on_vectors(dense_4x4_smooth):
+    """The coefficient array is an input of the recipe: with the min-max coefficients the polynomial sign function stays
+    within ITS (smaller) delta of the exact dense sign - uniformly in eta, which the operator norm on the
+    dense spectrum checks."""
+    d4 = dense_4x4_smooth
+    lam, W, Qmat = d4["lam"], d4["W"], d4["Qmat"]
+    shape = tuple(d4["dims"]) + (4, 3)
+    Q = lambda v: (Qmat @ v.reshape(-1)).reshape(shape)
+    eta = gaussian_spinor(d4["dims"])
+    qnorm = 6.4
+    eps = 0.99 * (lam ** 2).min() / qnorm ** 2
+    S = ((W * np.sign(lam)) @ W.conj().T @ eta.reshape(-1)).reshape(shape)
+    n = 40
+    errs = {}
+    for name, (c, delta) in {"minmax": sign.minmax_coeffs(n, eps)[:2], "interp": (sign.cheb_coeffs(n, eps), None)}.items():
+        delta = sign.measure_delta(c, eps) if delta is None else delta
+        errs[name] = np.linalg.norm((sign.sign_poly(Q, eta, c, eps, qnorm) - S).ravel()) / np.linalg.norm(eta.ravel())
+        assert errs[name] <= delta
+        x = lam / qnorm
+        assert np.abs(x * sign.eval_P_scalar(c, eps, x * x) - np.sign(x)).max() <= delta      # || X P(X^2) - sign Q || <= delta
