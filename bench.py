@@ -23,9 +23,10 @@ configs  = the other timed BASELINE.json configurations, driver-run in the same 
 cpu_baseline / --impl reference = the CPU oracle (oracle/, plain C + numpy, as it stands) on the host cores on a
            bounded sample of the same workload.
 
-Multi-GPU: `--gpus N` runs N independent replicas (one lattice per GPU, different sources), no
-data-path collective, scaling = weak; when not started by torchrun it starts the N ranks itself.  Timing: barrier +
-synchronize, CUDA events, max over ranks.
+Multi-GPU: `--gpus N` splits the SAME 32^3x64 lattice along x0 over the N GPUs (domain decomposition,
+csrc/shard.cu: two half-spinor faces per stencil over NCCL / NVLink, global reductions by all-reduce), scaling = strong;
+`--replicas` runs N independent lattices instead (no data-path collective, scaling = weak).  When not started by torchrun the
+script starts the N ranks itself.  Timing: barrier + synchronize, CUDA events, max over ranks.
 """
 import argparse
 import json
@@ -167,7 +168,8 @@ def max_over_ranks(ms, world, backend_device=None):
 
 
 def whole_job_value(units_per_rank, world, ms):
-    """value = the units ALL ranks processed / the max-over-ranks time (weak scaling, replicas)."""
+    """value = the units ALL ranks processed / the max-over-ranks time (replicas: every rank does units_per_rank; domain
+    decomposition: units_per_rank is the rank's share of the one global lattice)."""
     return units_per_rank * world / (ms * 1e-3)
 
 
@@ -466,15 +468,26 @@ def run_b200(args):
         import torch.distributed as dist
 
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    dims = parse_lattice(args.lattice)
+    gdims = parse_lattice(args.lattice)
     prec, recon, n, l = args.prec, args.recon, args.degree, args.lowmodes
     peak, peak_src = load_peaks()
 
     # BASELINE config index 2: Haar-random links, seeded (--field smooth for the exp(i eps H) recipe)
-    U64 = gauge_field(dims, args.field, eps=args.field_eps)
+    U64 = gauge_field(gdims, args.field, eps=args.field_eps)
+    decompose = world > 1 and not args.replicas
+    if decompose:
+        # domain decomposition: this rank's time-slices of the one global lattice (nd_shard_layout), faces over NCCL
+        from paper_1010_5636_b200.dist import TorchDistComm
+
+        tb, tl, _, _ = nd.shard_layout(gdims[0], world, rank)
+        dims = (tl,) + tuple(gdims[1:])
+        Uloc = np.ascontiguousarray(U64[:, tb:tb + tl])
+    else:
+        dims, Uloc = gdims, U64
     ctx = nd.Context(dims, prec=prec, recon=recon, bc_time=-1, device=local)
-    ctx.set_gauge(U64.astype(np.complex64) if prec == 32 else U64)
-    V = ctx.V
+    ctx.set_gauge(Uloc.astype(np.complex64) if prec == 32 else Uloc)
+    comm = TorchDistComm(ctx) if decompose else None      # from here on every call acts on the global lattice
+    V = ctx.V                                             # sites of this rank
     c, delta = nd.cheb_coeffs(n, args.eps)
     ctx.set_sign_poly(c, args.eps, QNORM, M_KERNEL)
     eig = None
@@ -499,8 +512,8 @@ def run_b200(args):
         modes, nu = build_modes(ctx, l)
     ctx.set_lowmodes(modes, nu)
     eta, out, work = ctx.new_spinor(), ctx.new_spinor(), ctx.new_spinor(3)
-    ctx.gaussian(eta, 5636 + rank)                        # replicas: a different source per rank
-    step = lambda: ctx.apply_DN(out, eta, 1.0 / RHO, work, use_graph=True)
+    ctx.gaussian(eta, 5636 + (0 if decompose else rank))  # replicas: a different source per rank
+    step = lambda: ctx.apply_DN(out, eta, 1.0 / RHO, work, use_graph=True)   # (no graph while sharded: host callbacks)
 
     # ---- device-resident leg
     for _ in range(args.warmup):
@@ -551,22 +564,25 @@ def run_b200(args):
             dist.destroy_process_group()
         return
     # ---- rank 0 only: the dominant kernel alone (roofline), every variant; layout; the other configs; the CPU oracle
+    # (single-GPU legs on the global lattice; the other ranks wait at the final barrier)
     ctx.close()
-    del modes, eta, out, work
+    del modes, eta, out, work, comm
     torch.cuda.empty_cache()
+    dims = gdims
+    V_global = int(np.prod(gdims))
     qk = {}
     q_sampler = ClockSampler(local).start()
     for p, r in ((32, 12), (64, 12), (32, 8), (64, 8), (32, 18), (64, 18)):
         if args.quick and (p, r) != (prec, recon):
             continue
         variants = (None, "site", "tile_tma") if p == 32 else (None,)
-        qk[f"f{p}_recon{r}"] = measure_q_kernel(torch, nd, dims, args.lattice, U64, p, r, peak, variants)
+        qk[f"f{p}_recon{r}"] = measure_q_kernel(torch, nd, gdims, args.lattice, U64, p, r, peak, variants)
     q_clocks = q_sampler.stop()
     main = qk[f"f{prec}_recon{recon}"]
     roofline = {"bound": "hbm", "achieved": main["achieved_gbs"], "peak": peak, "unit": "GB/s",
                 "frac": main["achieved_gbs"] / peak, "traffic": main["dram_traffic_ncu"],
                 "kernel": f"{main['kernel']} (Q stencil, plain epilogue; stencil variant '{main['stencil_variant']}')",
-                "peak_source": peak_src, "algorithmic_bytes_per_launch": main["bytes_per_site"] * V,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": main["bytes_per_site"] * V_global,
                 "us_per_launch": main["us_per_launch"], "timing": "median of 5 batches of 20 launches, CUDA events on the launch stream",
                 "frac_of_8TBs_nominal": main["achieved_gbs"] / 8000.0, "clocks": q_clocks,
                 "traffic_source": "profiles/q_kernel_dram_traffic.csv (ncu --set full of this kernel on this lattice; null = no capture)"}
@@ -584,17 +600,18 @@ def run_b200(args):
         cpu = cpu_baseline_sample(dims=(32, 16, 16, 16), n=6)
     line = {
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if decompose else "weak", "vs_baseline": None,
         "dtype": "f32" if prec == 32 else "f64", "data": "synthetic",
         "config": {"workload": f"D_N apply (eq. 2.4+2.11) on {args.lattice}, {args.field} SU(3) links, m=-1.6, recon {recon}, "
                                f"degree n={n} (2n+1={stencils} Q stencils), l={l} projected vectors, CUDA graph",
-                   "lattice": args.lattice, "sites": V, "recon": recon, "degree": n, "eps": args.eps, "delta": delta,
-                   "lowmodes": l, "lowmodes_kind": modes_kind, "stencil_variant": headline_variant,
-                   "replicas": world, "parallelism": f"replicas x{world}",
+                   "lattice": args.lattice, "sites": V_global, "sites_per_gpu": V, "recon": recon, "degree": n, "eps": args.eps,
+                   "delta": delta, "lowmodes": l, "lowmodes_kind": modes_kind, "stencil_variant": headline_variant,
+                   "parallelism": (f"domain decomposition along x0 over {world} GPUs ({gdims[0] // world} slices each), "
+                                   f"half-spinor faces over NCCL" if decompose else f"replicas x{world}"),
                    "l2_policy": "inputs larger than L2 (links + vectors >= 1.4 GB fp32), no flush needed"},
-        "dn_applies_per_s": world * args.steps / (ms * 1e-3),
-        "q_stencils_per_s": world * args.steps * stencils / (ms * 1e-3),
-        "tau_ns_per_clenshaw_iteration_per_site": ms * 1e6 / args.steps / (n * V),
+        "dn_applies_per_s": (1 if decompose else world) * args.steps / (ms * 1e-3),
+        "q_stencils_per_s": (1 if decompose else world) * args.steps * stencils / (ms * 1e-3),
+        "tau_ns_per_clenshaw_iteration_per_site": ms * 1e6 / args.steps / (n * V * (world if decompose else 1)),
         "tau_paper_ns": {"single_GTX285": 38.0, "double_GTX285": 90.0, "source": "PAPER.md:L140-142 (context, other hardware)"},
         "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": hbytes, "d2h_bytes_per_step": hbytes,
                 "ms_per_step": ms_e2e / args.steps},
@@ -659,6 +676,7 @@ def main():
     ap.add_argument("--eig-degree", type=int, default=100)
     ap.add_argument("--quick", action="store_true", help="headline + its own Q-kernel variant only (no layout / configs legs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--replicas", action="store_true", help="--gpus N as N independent lattices (weak scaling) instead of the domain decomposition")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:

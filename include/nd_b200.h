@@ -212,6 +212,34 @@ ND_API int nd_projector_error(int l, const double* nu, const double* rho, int nr
  * Jacobi method: a = Z diag(w) Z^dagger, w[k] ascending, eigenvector j in COLUMN j of z (row-major, k*k complex). */
 ND_API int nd_heev(int k, const double* a, double* w, double* z);
 
+/* ------------------------------------------------------------------------------------ domain decomposition
+ * The lattice split along x0 (time) over nranks GPUs, one process per GPU: rank r owns
+ * the slices [r T/nranks, (r+1) T/nranks) as a context created with the LOCAL dims (T/nranks, L1, L2, L3) and the GLOBAL
+ * bc_time, its local links set by nd_set_gauge, then nd_set_sharding.  From then on every operator call of this header acts
+ * on the rank's part of the global field and every reduction returns the GLOBAL value; all ranks must make the same calls in
+ * the same order.  Per stencil application each rank sends two faces of projected half-spinors (nd_halo_bytes each; the face
+ * for the next rank already multiplied by U_0^dagger, so links never travel; bc_time applied where a face crosses the global
+ * seam) while the local stencil runs, and adds the two received hops to its boundary slices.  The transfers are the
+ * caller's, through callbacks that work on DEVICE pointers owned by the context (valid until nd_destroy / the next
+ * nd_set_sharding) and must be ordered with the context's stream:
+ *   start(user, send_next, send_prev, recv_prev, recv_next, bytes): begin  send_next -> next rank's recv_prev,
+ *                                                                          send_prev -> previous rank's recv_next
+ *   wait(user):            the context's stream must not run past this point before both recv buffers are complete
+ *   allreduce(user, d_buf, n): sum n doubles in device memory over the ranks, in place, ordered with the stream
+ * (return 0 on success).  paper_1010_5636_b200/dist.py implements them with torch.distributed (NCCL send/recv over NVLink).
+ * nranks == 1 removes the sharding.  CUDA graphs are not used while sharded.
+ * nd_shard_layout (host helper, no GPU): first global slice and local extent of a rank, and whether its previous / next
+ * face crosses the global seam; ND_ERR_BAD_ARG unless nranks divides T into parts of at least 2 slices. */
+typedef int (*nd_exchange_start_fn)(void* user, const void* send_next, const void* send_prev, void* recv_prev, void* recv_next,
+                                    size_t bytes);
+typedef int (*nd_exchange_wait_fn)(void* user);
+typedef int (*nd_allreduce_fn)(void* user, double* d_buf, int n);
+ND_API int nd_shard_layout(int T, int nranks, int rank, int* t_begin, int* t_local, int* crosses_seam_prev, int* crosses_seam_next);
+ND_API int nd_set_sharding(nd_ctx* ctx, int rank, int nranks, nd_exchange_start_fn start, nd_exchange_wait_fn wait,
+                           nd_allreduce_fn allreduce, void* user);
+ND_API size_t nd_halo_bytes(const nd_ctx* ctx);   /* bytes of one face: (V_local / T_local) * 12 reals */
+ND_API int nd_halo_buffers(nd_ctx* ctx, void** send_next, void** send_prev, void** recv_prev, void** recv_next);
+
 /* ------------------------------------------------------------------------------------------------ BLAS-1
  * Spinor-field vector operations (device SoA).  a = (re, im).
  *   nd_axpy:       y <- a x + y            nd_scale: x <- a x         nd_copy: y <- x

@@ -35,6 +35,11 @@ SIGNATURES = {
     "nd_spinor_bytes": (_c_sz, [_c_vp]),
     "nd_gauge_bytes": (_c_sz, [_c_vp]),
     "nd_launch_count": (_c_ll, [_c_vp]),
+    "nd_shard_layout": (_c_int, [_c_int, _c_int, _c_int, ctypes.POINTER(_c_int), ctypes.POINTER(_c_int), ctypes.POINTER(_c_int),
+                                 ctypes.POINTER(_c_int)]),
+    "nd_set_sharding": (_c_int, [_c_vp, _c_int, _c_int, _c_vp, _c_vp, _c_vp, _c_vp]),
+    "nd_halo_bytes": (_c_sz, [_c_vp]),
+    "nd_halo_buffers": (_c_int, [_c_vp, ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp)]),
     "nd_set_stencil_variant": (_c_int, [_c_vp, _c_int]),
     "nd_get_stencil_variant": (_c_int, [_c_vp]),
     "nd_set_gauge": (_c_int, [_c_vp, _c_vp, _c_int, _c_int]),
@@ -77,6 +82,10 @@ SIGNATURES = {
     "nd_norm2_dev": (_c_int, [_c_vp, _c_vp, _c_vp]),
     "nd_gaussian": (_c_int, [_c_vp, _c_vp, _c_ull]),
 }
+
+EXCHANGE_START_FN = ctypes.CFUNCTYPE(_c_int, _c_vp, _c_vp, _c_vp, _c_vp, _c_vp, _c_sz)
+EXCHANGE_WAIT_FN = ctypes.CFUNCTYPE(_c_int, _c_vp)
+ALLREDUCE_FN = ctypes.CFUNCTYPE(_c_int, _c_vp, _c_vp, _c_int)
 
 _lib = None
 
@@ -157,6 +166,16 @@ def projector_error(nu, rho, rest):
     if rc != ND_OK:
         raise NDError(rc, "nd_projector_error")
     return kappa, bound, d
+
+
+def shard_layout(T, nranks, rank):
+    """nd_shard_layout: (t_begin, t_local, crosses_seam_prev, crosses_seam_next) - host utility, needs no GPU."""
+    lib = load_library()
+    tb, tl, cp, cn = _c_int(0), _c_int(0), _c_int(0), _c_int(0)
+    rc = lib.nd_shard_layout(int(T), int(nranks), int(rank), ctypes.byref(tb), ctypes.byref(tl), ctypes.byref(cp), ctypes.byref(cn))
+    if rc != ND_OK:
+        raise NDError(rc, "nd_shard_layout")
+    return tb.value, tl.value, bool(cp.value), bool(cn.value)
 
 
 def choose_l(abs_nu, l_min, l_max):
@@ -240,6 +259,52 @@ class Context:
         shape = (24 * self.V,) if count is None else (int(count), 24 * self.V)
         with torch.cuda.stream(self.stream):
             return torch.empty(shape, dtype=self.real_dtype, device=self.torch_device)
+
+    # -- domain decomposition
+    def set_sharding(self, rank, nranks, start=None, wait=None, allreduce=None):
+        """start(send_next, send_prev, recv_prev, recv_next, bytes), wait(), allreduce(d_buf, n): Python callables working on
+        raw device pointers (ints); exceptions become a non-zero status.  nranks = 1 removes the sharding."""
+        def guard(fn):
+            def call(*a):
+                try:
+                    fn(*a[1:])          # drop the unused `user` pointer
+                    return 0
+                except Exception:       # a callback must not unwind into C
+                    import traceback
+
+                    traceback.print_exc()
+                    return 1
+            return call
+
+        if nranks > 1:
+            self._cb = (EXCHANGE_START_FN(guard(start)), EXCHANGE_WAIT_FN(guard(wait)), ALLREDUCE_FN(guard(allreduce)))
+            self._chk(self.lib.nd_set_sharding(self._h, int(rank), int(nranks), ctypes.cast(self._cb[0], _c_vp),
+                                               ctypes.cast(self._cb[1], _c_vp), ctypes.cast(self._cb[2], _c_vp), None))
+        else:
+            self._chk(self.lib.nd_set_sharding(self._h, 0, 1, None, None, None, None))
+            self._cb = None
+
+    def halo_bytes(self):
+        return int(self.lib.nd_halo_bytes(self._h))
+
+    def halo_buffers(self):
+        """(send_next, send_prev, recv_prev, recv_next) device pointers."""
+        p = [_c_vp() for _ in range(4)]
+        self._chk(self.lib.nd_halo_buffers(self._h, *[ctypes.byref(x) for x in p]))
+        return tuple(int(x.value) for x in p)
+
+    def wrap_device_memory(self, ptr, nbytes, dtype):
+        """A torch tensor aliasing `nbytes` of device memory at `ptr` (owned by the library)."""
+        torch = self._torch
+
+        class _Raw:
+            pass
+
+        raw = _Raw()
+        itemsize = torch.empty((), dtype=dtype).element_size()
+        typestr = {torch.float32: "<f4", torch.float64: "<f8", torch.uint8: "|u1"}[dtype]
+        raw.__cuda_array_interface__ = {"shape": (nbytes // itemsize,), "typestr": typestr, "data": (int(ptr), False), "version": 2}
+        return torch.as_tensor(raw, device=self.torch_device)
 
     STENCIL = {"auto": 0, "site": 1, "tile": 2, "tile_tma": 3}
 

@@ -79,6 +79,14 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->tile_ok = ndi_tile_supported(ctx);
     ctx->stencil_variant = ND_STENCIL_AUTO;
     ctx->dot_configured = false;
+    ctx->shard_rank = 0;
+    ctx->shard_n = 1;
+    ctx->in_shard_call = false;
+    for (int i = 0; i < 4; i++) ctx->halo[i] = nullptr;
+    ctx->exchange_start = nullptr;
+    ctx->exchange_wait = nullptr;
+    ctx->allreduce = nullptr;
+    ctx->comm_user = nullptr;
     // fp32 recon 18 is stored as 9 float2, everything else in 128-bit words: bytes = 4 * recon * V * prec/8
     ctx->gauge_bytes = (size_t)4 * recon * ctx->V * (prec / 8);
     cudaError_t e = cudaMalloc(&ctx->gauge, ctx->gauge_bytes);
@@ -112,6 +120,8 @@ extern "C" int nd_destroy(nd_ctx* ctx) {
     if (ctx->d_coef) cudaFree(ctx->d_coef);
     if (ctx->d_nu) cudaFree(ctx->d_nu);
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
+    for (int i = 0; i < 4; i++)
+        if (ctx->halo[i]) cudaFree(ctx->halo[i]);
     delete ctx;
     return ND_OK;
 }

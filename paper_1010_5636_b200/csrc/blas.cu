@@ -345,10 +345,10 @@ __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned
 }
 // word index w -> 4 (fp32) or 2 (fp64) standard normals by Box-Muller
 template <typename T>
-__global__ void gaussian_kernel(typename Prec<T>::Vec* __restrict__ x, unsigned long long seed, long long nwords) {
+__global__ void gaussian_kernel(typename Prec<T>::Vec* __restrict__ x, unsigned long long seed, long long nwords, unsigned shard) {
     for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < nwords; w += (long long)gridDim.x * blockDim.x) {
         unsigned r[4];
-        philox4x32_10((unsigned)w, (unsigned)(w >> 32), 0u, 0u, (unsigned)seed, (unsigned)(seed >> 32), r);
+        philox4x32_10((unsigned)w, (unsigned)(w >> 32), shard, 0u, (unsigned)seed, (unsigned)(seed >> 32), r);   // counter = (word, shard rank)
         typename Prec<T>::Vec o;
         T* po = reinterpret_cast<T*>(&o);
         if (sizeof(T) == 4) {
@@ -413,7 +413,7 @@ int block_dot_cols_t(nd_ctx* ctx, int l, const void* v, int nc, const void* cons
         reduce_partials_kernel<<<n * l * 2, RED_THREADS, 0, ctx->stream>>>(d_out + (size_t)2 * l * c0, ctx->d_partial, (int)blocks);
         ND_LAUNCHED(ctx);
     }
-    return ND_OK;
+    return ndi_allreduce(ctx, d_out, 2 * l * nc);   // domain decomposition: the local sums become global ones
 }
 
 }  // namespace
@@ -468,7 +468,8 @@ int ndi_block_resid(nd_ctx* ctx, int k, const void* x, const void* y, const doub
     ND_LAUNCHED(ctx);
     reduce_partials_kernel<<<k, RED_THREADS, 0, ctx->stream>>>(ctx->d_result, ctx->d_partial, (int)bx);
     ND_LAUNCHED(ctx);
-    int rc = ndi_read_result(ctx, ctx->d_result, rho, k);
+    int rc = ndi_allreduce(ctx, ctx->d_result, k);
+    if (rc == ND_OK) rc = ndi_read_result(ctx, ctx->d_result, rho, k);
     for (int i = 0; i < k && rc == ND_OK; i++) rho[i] = sqrt(rho[i] > 0.0 ? rho[i] : 0.0);
     return rc;
 }
@@ -594,8 +595,8 @@ extern "C" int nd_gaussian(nd_ctx* ctx, void* x, unsigned long long seed) {
     if (!x) return nd_fail(ctx, ND_ERR_BAD_ARG, "gaussian: null argument");
     const long long nwords = ctx->V * (ctx->prec == 32 ? 6 : 12);
     const unsigned blocks = grid_for(nwords, 256, 1 << 30);
-    if (ctx->prec == 32) gaussian_kernel<float><<<blocks, 256, 0, ctx->stream>>>((float4*)x, seed, nwords);
-    else gaussian_kernel<double><<<blocks, 256, 0, ctx->stream>>>((double2*)x, seed, nwords);
+    if (ctx->prec == 32) gaussian_kernel<float><<<blocks, 256, 0, ctx->stream>>>((float4*)x, seed, nwords, (unsigned)ctx->shard_rank);
+    else gaussian_kernel<double><<<blocks, 256, 0, ctx->stream>>>((double2*)x, seed, nwords, (unsigned)ctx->shard_rank);
     ND_LAUNCHED(ctx);
     return ND_OK;
 }

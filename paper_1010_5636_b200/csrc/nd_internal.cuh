@@ -64,6 +64,14 @@ struct nd_ctx {
     bool tile_ok;               // the tiled marching stencil (wilson_tile.cu) takes this lattice
     int stencil_variant;        // ND_STENCIL_* (nd_set_stencil_variant)
     int tile_ctas_per_sm[4];    // resident CTAs per SM of the tiled kernel ({cp.async, TMA} x {plain, fused}), 0 = not queried yet
+    // domain decomposition along x0 (shard.cu): this context is the local lattice of rank shard_rank of shard_n
+    int shard_rank, shard_n;
+    bool in_shard_call;         // the local stencil of a sharded application is being enqueued
+    void* halo[4];              // send_next, send_prev, recv_prev, recv_next: half-spinor faces (nd_halo_bytes each)
+    nd_exchange_start_fn exchange_start;
+    nd_exchange_wait_fn exchange_wait;
+    nd_allreduce_fn allreduce;
+    void* comm_user;
     char err[512];
 };
 
@@ -161,6 +169,9 @@ int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi,
                      const void* v2, double s3, const void* v3);
 int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
                       double s2, const void* v2, double s3, const void* v3);
+int ndi_halo_pack(nd_ctx* ctx, const void* in);                 // faces of `in` -> halo[0], halo[1]
+int ndi_halo_apply(nd_ctx* ctx, void* out, double s0);          // halo[2], halo[3] -> the boundary slices of out
+int ndi_allreduce(nd_ctx* ctx, double* d_buf, int n);           // sum over ranks (no-op unless sharded)
 int ndi_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out);   // d_out: 2l doubles (device)
 int ndi_block_dot_cols_dev(nd_ctx* ctx, int l, const void* v, int nc, const void* const* cols, double* d_out);   // d_out[(c*l+k)*2+ri]
 int ndi_block_axpy_batch_dev(nd_ctx* ctx, int l, int nb, const double* d_coef, const void* v, void* y, int mode, const void* eta,

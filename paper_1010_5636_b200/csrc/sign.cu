@@ -112,7 +112,7 @@ int apply_sign_impl(nd_ctx* ctx, int nb, void* out, const void* in, void* work, 
     if (!ctx->gauge_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_sign/DN: gauge field not set");
     if (!ctx->poly_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "apply_sign/DN: polynomial not set (nd_set_sign_poly)");
     ND_CUDA(ctx, cudaSetDevice(ctx->device));
-    if (!use_graph || ctx->stream == nullptr) return enqueue_sign(ctx, nb, out, in, work, kind, pa, pb);
+    if (!use_graph || ctx->stream == nullptr || ctx->shard_n > 1) return enqueue_sign(ctx, nb, out, in, work, kind, pa, pb);
     for (auto& g : ctx->graphs)
         if (g.out == out && g.in == in && g.work == work && g.kind == kind && g.pa == pa && g.pb == pb && g.nrhs == nb) {
             ND_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));

@@ -296,6 +296,30 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
     }
     // the tiled marching kernel (wilson_tile.cu) where it is the faster one: fp32 on lattices it supports; with the
     // uncompressed recon-18 links (64-bit words in fp32) only the fused-epilogue variant wins (224 vs 199 us plain, 252 vs 276 us fused)
+    if (ctx->shard_n > 1 && !ctx->in_shard_call) {
+        // domain decomposition (shard.cu): faces out, the local stencil with the wrapped time hops switched off while the
+        // transfer runs, faces in.  One right-hand side at a time (the halo buffers hold one face pair).
+        const size_t sb = nd_spinor_bytes(ctx);
+        for (int j = 0; j < nrhs; j++) {
+            const size_t o = (size_t)j * sb;
+            int rc = ndi_halo_pack(ctx, (const char*)in + o);
+            if (rc != ND_OK) return rc;
+            if (ctx->exchange_start(ctx->comm_user, ctx->halo[0], ctx->halo[1], ctx->halo[2], ctx->halo[3], nd_halo_bytes(ctx)) != 0)
+                return nd_fail(ctx, ND_ERR_CUDA, "sharding: the exchange-start callback failed");
+            ctx->in_shard_call = true;
+            const int saved_bc = ctx->bc;
+            ctx->bc = 0;   // phase of the hops across the local time boundary: they come from the neighbours instead
+            rc = ndi_apply_Q_batch(ctx, 1, (char*)out + o, (const char*)in + o, m, epi, s0, s1, v1 ? (const char*)v1 + o : nullptr, s2,
+                                   v2 ? (const char*)v2 + o : nullptr, s3, v3 ? (const char*)v3 + o : nullptr);
+            ctx->bc = saved_bc;
+            ctx->in_shard_call = false;
+            if (rc != ND_OK) return rc;
+            if (ctx->exchange_wait(ctx->comm_user) != 0) return nd_fail(ctx, ND_ERR_CUDA, "sharding: the exchange-wait callback failed");
+            rc = ndi_halo_apply(ctx, (char*)out + o, epi ? s0 : 1.0);
+            if (rc != ND_OK) return rc;
+        }
+        return ND_OK;
+    }
     const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->recon != 18 || epi))
                                                                 : (ctx->stencil_variant != ND_STENCIL_SITE);
     if (tile) {   // large lattices: one launch per right-hand side already fills the machine
