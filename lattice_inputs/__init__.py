@@ -14,6 +14,7 @@ from .generators import (  # noqa: F401
     SEED_GAUGE,
     SEED_SOURCE,
     SEED_TRANSFORM,
+    flux_su3,
     gaussian_spinor,
     gauge_field,
     haar_su3,

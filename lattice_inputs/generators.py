@@ -69,6 +69,30 @@ def gauge_field(dims, kind, seed=SEED_GAUGE, eps=0.3):
     return u.reshape((4,) + dims + (3, 3))
 
 
+def flux_su3(dims, q01, q23, noise=0.0, seed=SEED_GAUGE):
+    """A topologically non-trivial SU(3) field for the index tests: constant abelian field strength on the 4-torus in the
+    Cartan direction T = diag(1, -1, 0), with q01 flux quanta through the (x0, x1) planes and q23 through the (x2, x3)
+    planes (F = 2 pi q / (L_a L_b) per plaquette; the transition functions sit on the last links of x0 and x2), times an
+    optional random rotation exp(i noise H) of every link that removes the degeneracies of the purely diagonal field.
+    Input recipe only: diagonal phases and a matrix exponential, no operator of the method."""
+    dims = tuple(int(d) for d in dims)
+    L0, L1, L2, L3 = dims
+    t = np.array([1.0, -1.0, 0.0])
+    x = np.indices(dims)
+    f01 = 2.0 * np.pi * q01 / (L0 * L1)
+    f23 = 2.0 * np.pi * q23 / (L2 * L3)
+    phases = [np.where(x[0] == L0 - 1, -f01 * L0 * x[1], 0.0), f01 * x[0],
+              np.where(x[2] == L2 - 1, -f23 * L2 * x[3], 0.0), f23 * x[2]]
+    u = np.zeros((4,) + dims + (3, 3), dtype=np.complex128)
+    for mu in range(4):
+        for a in range(3):
+            u[mu, ..., a, a] = np.exp(1j * phases[mu] * t[a])
+    if noise:
+        r = smooth_su3(4 * int(np.prod(dims)), noise, _rng(seed)).reshape(u.shape)
+        u = np.einsum("...ij,...jk->...ik", r, u)
+    return u
+
+
 def gaussian_spinor(dims, seed=SEED_SOURCE):
     """psi[x0, x1, x2, x3, spin, colour], Re/Im ~ N(0,1)."""
     dims = tuple(int(d) for d in dims)
