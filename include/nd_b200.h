@@ -212,6 +212,27 @@ ND_API int nd_projector_error(int l, const double* nu, const double* rho, int nr
  * Jacobi method: a = Z diag(w) Z^dagger, w[k] ascending, eigenvector j in COLUMN j of z (row-major, k*k complex). */
 ND_API int nd_heev(int k, const double* a, double* w, double* z);
 
+/* ------------------------------------------------------------------------------------------------- index
+ * nd_index_count: the index of D_N by zero-mode counting (section 4).  D_N = c (1 + gamma5 sign(Q)) obeys the
+ * Ginsparg-Wilson relation, so D_N^dagger D_N commutes with gamma5 and every zero mode has chirality +1 or -1;
+ *     index = n_+ - n_-,   n_sigma = dim ker B_sigma,   B_sigma = P_sigma (1 + gamma5 sign(Q)) P_sigma = D_N^dagger D_N / (2 c^2)
+ * on the sector gamma5 = sigma, P_sigma = (1 + sigma gamma5)/2, spectrum in [0, 2].  For each sigma the nvec lowest eigenvalues
+ * of B_sigma are computed by Chebyshev-filtered block subspace iteration (filter degree `degree` per outer iteration, every
+ * application of B_sigma = one sign-function application with the polynomial and low modes set in the context, 2n+1 stencils)
+ * and a Rayleigh-Ritz step; a Ritz pair (theta_j, r_j = ||B x_j - theta_j x_j||) counts as a zero mode when
+ * theta_j + r_j <= zero_tol and as a non-zero mode when theta_j - r_j > zero_tol; the iteration stops when every pair of the
+ * block is decided and the lowest non-zero pair is located to 10 % (r_j <= 0.1 theta_j: the block sits on the low end).  zero_tol must sit between the sign function's error (delta, kappa_+-: the computed zero eigenvalues are
+ * O(delta)) and the lowest non-zero eigenvalue of B_sigma.
+ *   counts   [out, host]  (n_+, n_-)
+ *   evals, resid [out, host]  2*nvec values each: theta_j and r_j of sector +1, then of sector -1, ascending in theta
+ *   work     [device]  nd_index_work_spinors(nvec) = 3 nvec + 5 spinors
+ *   stats    (may be NULL) [0] outer iterations (both sectors), [1] sign-function applications
+ * Errors: ND_ERR_BAD_STATE without gauge field / polynomial; ND_ERR_NO_CONVERGENCE when a sector is undecided after maxit outer
+ * iterations; ND_ERR_BAD_ARG when all nvec vectors of a sector come out as zero modes (nvec must exceed n_sigma). */
+ND_API int nd_index_count(nd_ctx* ctx, int nvec, int degree, double zero_tol, int maxit, unsigned long long seed, int counts[2],
+                          double* evals, double* resid, void* work, long long* stats);
+ND_API size_t nd_index_work_spinors(int nvec);
+
 /* ------------------------------------------------------------------------------------ domain decomposition
  * The lattice split along x0 (time) over nranks GPUs, one process per GPU: rank r owns
  * the slices [r T/nranks, (r+1) T/nranks) as a context created with the LOCAL dims (T/nranks, L1, L2, L3) and the GLOBAL

@@ -66,6 +66,9 @@ SIGNATURES = {
     "nd_lowmodes_compute": (_c_int, [_c_vp, _c_int, _c_int, _c_int, _c_int, _c_dbl, _c_int, _c_dbl, _c_int, _c_ull, _c_vp, _pd, _pd,
                                      ctypes.POINTER(_c_int), _pd, _pd, _c_vp, ctypes.POINTER(_c_ll)]),
     "nd_lowmodes_work_spinors": (_c_sz, [_c_int, _c_int]),
+    "nd_index_count": (_c_int, [_c_vp, _c_int, _c_int, _c_dbl, _c_int, _c_ull, ctypes.POINTER(_c_int), _pd, _pd, _c_vp,
+                                ctypes.POINTER(_c_ll)]),
+    "nd_index_work_spinors": (_c_sz, [_c_int]),
     "nd_choose_l": (_c_int, [_c_int, _pd, _c_int, _c_int, ctypes.POINTER(_c_int), _pd]),
     "nd_projector_error": (_c_int, [_c_int, _pd, _pd, _c_int, _pd, _pd, _pd, _pd]),
     "nd_heev": (_c_int, [_c_int, _pd, _pd, _pd]),
@@ -475,6 +478,19 @@ class Context:
             iterations=int(stats[0]), stencils=int(stats[1]), converged=(rc == ND_OK), l_chosen=lp, kappa=kappa, bound=bound,
             nu_block=nu, rho_block=resid, nu_guard=nu[lp:].copy(), theta_rest=np.sort(nu[lp:] ** 2),
             message=(self.lib.nd_last_error(self._h).decode() if rc != ND_OK else ""))
+
+    def index_count(self, nvec, zero_tol, degree=8, maxit=40, seed=11):
+        """nd_index_count with the sign function set in the context -> (n_plus, n_minus, stats dict with the Ritz values
+        `evals` [2, nvec] and residues `resid` [2, nvec] of B_+ and B_-)."""
+        nvec = int(nvec)
+        work = self.new_spinor(int(self.lib.nd_index_work_spinors(nvec)))
+        counts = (_c_int * 2)()
+        evals, resid = np.zeros(2 * nvec), np.zeros(2 * nvec)
+        stats = (_c_ll * 2)()
+        self._chk(self.lib.nd_index_count(self._h, nvec, int(degree), float(zero_tol), int(maxit), int(seed), counts,
+                                          evals.ctypes.data_as(_pd), resid.ctypes.data_as(_pd), work.data_ptr(), stats))
+        return int(counts[0]), int(counts[1]), dict(evals=evals.reshape(2, nvec), resid=resid.reshape(2, nvec),
+                                                    iterations=int(stats[0]), sign_applications=int(stats[1]))
 
     # -- BLAS-1
     def axpy(self, a, x, y):

@@ -71,6 +71,27 @@ __global__ void gamma5_kernel(typename Prec<T>::Vec* y, const typename Prec<T>::
     }
 }
 
+// y <- P_sigma u + c y,  P_sigma = (1 + sigma gamma5)/2: keep the spin components of chirality sigma of u (0, 1 for +1; 2, 3 for -1),
+// zero the others (index by zero-mode counting: D_N^dagger D_N commutes with gamma5 and is diagonalised sector
+// by sector).  c == 0: y is not read.
+template <typename T>
+__global__ void chiral_combine_kernel(typename Prec<T>::Vec* y, const typename Prec<T>::Vec* u, int sigma, T c, long long V) {
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < V; s += (long long)gridDim.x * blockDim.x) {
+        cx<T> cu[12], cy[12];
+        load_site<T>(u, V, s, cu);
+        if (c != T(0)) load_site<T>(y, V, s, cy);
+        const int lo = (sigma > 0) ? 0 : 6;
+#pragma unroll
+        for (int i = 0; i < 12; i++) {
+            const bool keep = (i >= lo && i < lo + 6);
+            cx<T> r = keep ? cu[i] : cx<T>{T(0), T(0)};
+            if (c != T(0)) { r.re = fma(c, cy[i].re, r.re); r.im = fma(c, cy[i].im, r.im); }
+            cy[i] = r;
+        }
+        store_site<T>(y, V, s, cy);
+    }
+}
+
 // --------------------------------------------------------------------------------------- block dot product
 // <v_k, x_c> for k < l vectors of a block and up to NC columns x_c given by pointer (eq. 2.7 / 2.11: V^dagger psi; the
 // eigen-solver's Gram matrices).  Both operands move through HBM exactly once:
@@ -558,6 +579,14 @@ extern "C" int nd_gamma5(nd_ctx* ctx, void* y, const void* x) {
     ND_LAUNCHED(ctx);
     return ND_OK;
 }
+int ndi_chiral_combine(nd_ctx* ctx, int sigma, void* y, const void* u, double c) {
+    const unsigned blocks = (unsigned)std::min<long long>((ctx->V + 127) / 128, 8LL * ctx->num_sms);
+    if (ctx->prec == 32) chiral_combine_kernel<float><<<blocks, 128, 0, ctx->stream>>>((float4*)y, (const float4*)u, sigma, (float)c, ctx->V);
+    else chiral_combine_kernel<double><<<blocks, 128, 0, ctx->stream>>>((double2*)y, (const double2*)u, sigma, c, ctx->V);
+    ND_LAUNCHED(ctx);
+    return ND_OK;
+}
+
 extern "C" int nd_block_dot(nd_ctx* ctx, int l, const void* v, const void* x, double* out2l) {
     ND_ENTER(ctx);
     if (l < 1 || l > ND_MAX_BLOCK_L || !v || !x || !out2l) return nd_fail(ctx, ND_ERR_BAD_ARG, "block_dot: bad argument (1 <= l <= %d)", ND_MAX_BLOCK_L);

@@ -405,3 +405,163 @@ extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l_min, int l_max, int lguard
     }
     return finish(ND_OK);
 }
+
+// ------------------------------------------------------------------------ index by zero-mode counting
+// PAPER.md:L146 ("the calculation of the index of our Neuberger-Dirac operator via zero-mode counting").  D_N obeys the
+// Ginsparg-Wilson relation, so D_N^dagger D_N commutes with gamma5 and its zero modes have a definite chirality.  On the
+// sector gamma5 = sigma,
+//     D_N^dagger D_N / (2 c^2) = B_sigma = P_sigma (1 + gamma5 sign(Q)) P_sigma,   P_sigma = (1 + sigma gamma5)/2,
+// with spectrum in [0, 2].  For each sigma the lowest nvec eigenvalues of B_sigma are found by the block machinery above:
+//   X = nvec Gaussian vectors projected to the sector, orthonormalised
+//   repeat:  X_j <- p_d(B_sigma) X_j   (scaled Chebyshev recurrence, small on [cut, 2], 1 at the lowest Ritz value; one sign-
+//                                       function application = 2n+1 stencils per degree, nd_apply_DNm's launch sequence)
+//            orthonormalise;  Y = B_sigma X;  H = X^dagger Y = W diag(theta) W^dagger;  X <- X W, Y <- Y W;
+//            r_j = ||Y_j - theta_j X_j||: an eigenvalue of B_sigma lies within r_j of theta_j
+//   until every pair is decided: zero mode (theta_j + r_j <= zero_tol) or not (theta_j - r_j > zero_tol), the lowest pair
+//   that is not has r_j <= 0.1 theta_j (the block has converged onto the low end of the spectrum), and at least one pair is
+//   not a zero mode (else the block may be smaller than the kernel: ND_ERR_BAD_ARG, enlarge nvec).
+// n_sigma = number of zero modes of chirality sigma, index = n_+ - n_-.
+namespace {
+
+struct SectorOp {
+    Solver* S;
+    int sigma;
+    char* sw;          // 3 work spinors of the sign function
+    long long signs;   // sign-function applications
+    // out = P_sigma (pa in + pb gamma5 sign(Q) in) + pc out
+    int apply(void* out, const void* in, double pa, double pb, double pc, char* tmp) {
+        signs++;
+        int rc = ndi_apply_DNm(S->ctx, tmp, in, pa, pb, sw, 0);
+        if (rc != ND_OK) return rc;
+        return ndi_chiral_combine(S->ctx, sigma, out, tmp, pc);
+    }
+    // X_j <- p_d(B) X_j on [lo, hi] damped, normalised to 1 at `low` (the recurrence of Solver::filter with B for Q^2)
+    int filter(int d, double low, double lo, double hi) {
+        const double c = 0.5 * (hi + lo), e = 0.5 * (hi - lo);
+        const double sigma1 = e / (low - c);
+        for (int j = 0; j < S->k; j++) {
+            char* P = S->x(j);
+            char* R = S->s0;
+            // t_1 = (sigma_1/e)(B - c) t_0
+            int rc = apply(R, P, (1.0 - c) * sigma1 / e, sigma1 / e, 0.0, S->s1);
+            if (rc != ND_OK) return rc;
+            double sg = sigma1;
+            for (int i = 1; i < d; i++) {
+                const double sn = 1.0 / (2.0 / sigma1 - sg);
+                // t_{i+1} = (2 sn/e)(B - c) t_i - sg sn t_{i-1}, written over t_{i-1}
+                rc = apply(P, R, (1.0 - c) * 2.0 * sn / e, 2.0 * sn / e, -sg * sn, S->s1);
+                if (rc != ND_OK) return rc;
+                std::swap(P, R);
+                sg = sn;
+            }
+            // d even: t_d sits in x(j) again
+        }
+        return ND_OK;
+    }
+};
+
+}  // namespace
+
+extern "C" size_t nd_index_work_spinors(int nvec) { return (size_t)3 * nvec + 5; }
+
+extern "C" int nd_index_count(nd_ctx* ctx, int nvec, int degree, double zero_tol, int maxit, unsigned long long seed, int counts[2],
+                              double* evals, double* resid, void* work, long long* stats) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (nvec < 2 || nvec > ND_MAX_BLOCK_L || degree < 2 || maxit < 1 || !(zero_tol > 0.0 && zero_tol < 1.0) || !counts || !evals ||
+        !resid || !work)
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "index_count: bad argument (2 <= nvec <= %d, degree >= 2, 0 < zero_tol < 1)", ND_MAX_BLOCK_L);
+    if (!ctx->gauge_set || !ctx->poly_set) return nd_fail(ctx, ND_ERR_BAD_STATE, "index_count: gauge field / sign polynomial not set");
+    if (6 * ctx->V < nvec) return nd_fail(ctx, ND_ERR_BAD_ARG, "index_count: block larger than a chirality sector");
+    ND_CUDA(ctx, cudaSetDevice(ctx->device));
+    Solver S;
+    S.ctx = ctx;
+    S.sb = nd_spinor_bytes(ctx);
+    S.k = nvec;
+    S.m = ctx->m_sign;
+    S.stencils = 0;
+    const int k = nvec;
+    char* base = (char*)work;
+    S.s0 = base + (size_t)3 * k * S.sb;
+    S.s1 = S.s0 + S.sb;
+    S.d_mat = nullptr;
+    ND_CUDA(ctx, cudaMalloc((void**)&S.d_mat, (size_t)2 * k * k * sizeof(double)));
+    SectorOp B;
+    B.S = &S;
+    B.sw = S.s1 + S.sb;
+    B.signs = 0;
+    const int d = degree + (degree & 1);
+    long long its = 0;
+    auto finish = [&](int code) {
+        cudaFree(S.d_mat);
+        if (stats) { stats[0] = its; stats[1] = B.signs; }
+        return code;
+    };
+    std::vector<double> theta(k), z((size_t)2 * k * k), rho(k);
+    for (int sec = 0; sec < 2; sec++) {
+        B.sigma = (sec == 0) ? +1 : -1;
+        S.X = base;
+        S.Y = base + (size_t)k * S.sb;
+        S.Z = base + (size_t)2 * k * S.sb;
+        int rc = ND_OK;
+        for (int j = 0; j < k && rc == ND_OK; j++) {
+            rc = nd_gaussian(ctx, S.s0, seed + (unsigned long long)(sec * k + j));
+            if (rc == ND_OK) rc = ndi_chiral_combine(ctx, B.sigma, S.x(j), S.s0, 0.0);
+        }
+        if (rc == ND_OK) rc = S.orthonormalise();
+        if (rc != ND_OK) return finish(rc);
+        double cut = 2.0, low = 0.0;
+        bool decided = false;
+        int nzero = 0;
+        for (int it = 0; it <= maxit; it++) {
+            if (it > 0) {
+                rc = B.filter(d, low, cut, 2.0);
+                if (rc == ND_OK) rc = S.orthonormalise();
+                if (rc != ND_OK) return finish(rc);
+                its++;
+            }
+            for (int j = 0; j < k && rc == ND_OK; j++) rc = B.apply(S.y(j), S.x(j), 1.0, 1.0, 0.0, S.s1);
+            if (rc == ND_OK) rc = S.gram(S.X, k, S.Y, k);
+            if (rc == ND_OK) rc = nd_heev(k, S.h_mat.data(), theta.data(), z.data());
+            if (rc != ND_OK) return finish(rc == ND_ERR_NO_CONVERGENCE ? nd_fail(ctx, rc, "index_count: Jacobi eigen-solver did not converge") : rc);
+            std::vector<zc> W((size_t)k * k);
+            for (size_t i = 0; i < (size_t)k * k; i++) W[i] = zc(z[2 * i], z[2 * i + 1]);
+            rc = S.rotate(S.Z, k, S.X, k, W);
+            if (rc != ND_OK) return finish(rc);
+            std::swap(S.X, S.Z);
+            rc = S.rotate(S.Z, k, S.Y, k, W);
+            if (rc != ND_OK) return finish(rc);
+            std::swap(S.Y, S.Z);
+            rc = ndi_block_resid(ctx, k, S.X, S.Y, theta.data(), rho.data());
+            if (rc != ND_OK) return finish(rc);
+            nzero = 0;
+            int nrest = 0;
+            for (int j = 0; j < k; j++) {
+                evals[sec * k + j] = theta[j];
+                resid[sec * k + j] = rho[j];
+                if (theta[j] + rho[j] <= zero_tol) nzero++;
+                else if (theta[j] - rho[j] > zero_tol) nrest++;
+            }
+            // every pair decided, and the block has settled on the LOW end of the spectrum: the lowest non-zero pair is located
+            // to 10 % (a block of unconverged vectors has theta ~ 1 and residues ~ 0.3: "no zero modes" only by accident)
+            decided = (nzero + nrest == k) && nzero < k && rho[nzero] <= 0.1 * theta[nzero];
+            if (nzero == k) decided = true;   // reported below
+            if (decided || it == maxit) break;
+            // damp everything above the block's largest Ritz value next time; keep the damped interval off the lowest values
+            cut = std::max(theta[k - 1], 4.0 * zero_tol);
+            low = std::max(0.0, std::min(theta[0], 0.5 * cut));
+            if (!(cut < 1.9)) cut = 1.9;
+        }
+        counts[sec] = nzero;
+        if (!decided) {
+            nd_fail(ctx, ND_ERR_NO_CONVERGENCE, "index_count: sector %+d undecided after %d iterations (lowest Ritz value %.3e, residue %.3e, zero_tol %.3e)",
+                    B.sigma, maxit, theta[0], rho[0], zero_tol);
+            return finish(ND_ERR_NO_CONVERGENCE);
+        }
+        if (nzero == k) {
+            nd_fail(ctx, ND_ERR_BAD_ARG, "index_count: all %d vectors of sector %+d are zero modes: the block may be smaller than the kernel, enlarge nvec", k,
+                    B.sigma);
+            return finish(ND_ERR_BAD_ARG);
+        }
+    }
+    return finish(ND_OK);
+}

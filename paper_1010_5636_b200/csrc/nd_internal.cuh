@@ -183,6 +183,7 @@ int ndi_apply_DNm(nd_ctx* ctx, void* out, const void* in, double pa, double pb, 
 int ndi_block_gram_dev(nd_ctx* ctx, int l, const void* v, int nx, const void* x, double* d_out);      // d_out[(j*l+k)*2+c]
 int ndi_block_rotate_dev(nd_ctx* ctx, int l, const double* d_coef, const void* v, int ny, void* y);  // coef[(j*l+i)*2+c]
 int ndi_block_resid(nd_ctx* ctx, int k, const void* x, const void* y, const double* nu, double* rho);   // rho_j = ||y_j - nu_j x_j||
+int ndi_chiral_combine(nd_ctx* ctx, int sigma, void* y, const void* u, double c);   // y <- P_sigma u + c y
 int ndi_read_result(nd_ctx* ctx, const double* d_src, double* h_dst, int n);              // sync copy to host
 int ndi_drop_graphs(nd_ctx* ctx);
 constexpr int ND_RESULT_DOUBLES = 4 * ND_MAX_BLOCK_L;
