@@ -83,9 +83,9 @@ def load_traffic(kernel, lattice, prec, recon):
     return None
 
 
-def stencil_kernel_name(variant, sites):
+def stencil_kernel_name(variant, sites, prec=32):
     if variant in ("tile", "tile_tma"):
-        return "wilson_Q_tile_kernel"
+        return "wilson_Q_tile_kernel" if prec == 32 else "wilson_Q_tile2_kernel"
     return "wilson_Q_hop_kernel" if sites < 16384 else "wilson_Q_kernel"
 
 
@@ -251,7 +251,7 @@ def measure_q_kernel(torch, nd, dims, lattice, U64, prec, recon, peak, variants=
         name = ctx.get_stencil_variant()
         ms, batches = median_of_batches(torch, ctx, lambda: ctx.apply_Q(y, x, M_KERNEL), reps)
         gbs = q_bytes_per_site(prec, recon) * V / (ms * 1e-3) / 1e9
-        kernel = stencil_kernel_name(name, V)
+        kernel = stencil_kernel_name(name, V, prec)
         r = {"prec": prec, "recon": recon, "stencil_variant": name, "kernel": kernel, "us_per_launch": ms * 1e3,
              "us_per_launch_batches": [b * 1e3 for b in batches], "gflops_1320": FLOP_PER_SITE * V / (ms * 1e-3) / 1e9,
              "bytes_per_site": q_bytes_per_site(prec, recon), "achieved_gbs": gbs, "frac_of_measured_peak": gbs / peak,
@@ -259,6 +259,17 @@ def measure_q_kernel(torch, nd, dims, lattice, U64, prec, recon, peak, variants=
         if out is None:
             out = r                      # the first variant is the one the library picks (auto)
             out["other_variants"] = {}
+            # the same kernel with the Clenshaw update in its epilogue (a5: out = s0 Q(in) + s1 v1 + s2 v2 + s3 v3, out == v2):
+            # every second stencil of a D_N application; three more vector streams in the byte model
+            v = ctx.new_spinor(3)
+            for j in range(3):
+                ctx.gaussian(v[j], 77 + j)
+            msf, _ = median_of_batches(torch, ctx, lambda: ctx.apply_Q_axpbycz(v[1], x, M_KERNEL, 0.05, -0.9, v[0], -0.5, v[1], 0.01, v[2]), reps)
+            gbf = q_bytes_per_site(prec, recon, 3) * V / (msf * 1e-3) / 1e9
+            out["fused_epilogue"] = {"kernel": stencil_kernel_name("site" if (prec == 64 and var is None) else name, V, prec),
+                                     "us_per_launch": msf * 1e3, "bytes_per_site": q_bytes_per_site(prec, recon, 3),
+                                     "achieved_gbs": gbf, "frac_of_measured_peak": gbf / peak, "frac_of_8TBs": gbf / 8000.0}
+            del v
         else:
             out["other_variants"][name] = {k: r[k] for k in ("kernel", "us_per_launch", "achieved_gbs", "frac_of_measured_peak")}
     ctx.close()
@@ -343,7 +354,7 @@ def dn_config(torch, nd, index, lattice, prec, field_eps, l_window, guard, n, ei
          "sources": sources, "dn_applies_per_s": sources / (ms * 1e-3), "ms_per_dn": ms / sources,
          "gflops_1320": FLOP_PER_SITE * V * (2 * n + 1) * sources / (ms * 1e-3) / 1e9,
          "tau_ns_per_clenshaw_iteration_per_site": ms * 1e6 / sources / (n * V),
-         "kernel": stencil_kernel_name(ctx.get_stencil_variant(), V)}
+         "kernel": stencil_kernel_name(ctx.get_stencil_variant(), V, prec)}
     if nrhs > 1:
         nb = min(nrhs, sources)
         workb = ctx.new_spinor(3 * nb)
@@ -378,7 +389,7 @@ def q_config(torch, nd, lattice="16^3x32", field_eps=0.3, reps=1000):
         runs[f"f{prec}_recon{recon}"] = {"ms_for_1000": ms, "us_per_Q": ms * 1e3 / reps,
                                          "gflops_1320": FLOP_PER_SITE * V * reps / (ms * 1e-3) / 1e9,
                                          "model_gbs": q_bytes_per_site(prec, recon) * V * reps / (ms * 1e-3) / 1e9,
-                                         "kernel": stencil_kernel_name(ctx.get_stencil_variant(), V)}
+                                         "kernel": stencil_kernel_name(ctx.get_stencil_variant(), V, prec)}
         ctx.close()
         del x, y
     torch.cuda.empty_cache()
@@ -484,6 +495,12 @@ def run_b200(args):
         Uloc = np.ascontiguousarray(U64[:, tb:tb + tl])
     else:
         dims, Uloc = gdims, U64
+    if args.q_only:
+        # the stencil of one precision / recon alone (the command the ncu captures under profiles/ run)
+        variants = (None,) if args.variant is None else (args.variant,)
+        r = measure_q_kernel(torch, nd, gdims, args.lattice, U64, prec, recon, peak, variants, reps=args.steps)
+        print(json.dumps({"q_only": r, "lattice": args.lattice, "peak_gbs": peak, "peak_source": peak_src}))
+        return
     ctx = nd.Context(dims, prec=prec, recon=recon, bc_time=-1, device=local)
     ctx.set_gauge(Uloc.astype(np.complex64) if prec == 32 else Uloc)
     comm = TorchDistComm(ctx) if decompose else None      # from here on every call acts on the global lattice
@@ -575,7 +592,7 @@ def run_b200(args):
     for p, r in ((32, 12), (64, 12), (32, 8), (64, 8), (32, 18), (64, 18)):
         if args.quick and (p, r) != (prec, recon):
             continue
-        variants = (None, "site", "tile_tma") if p == 32 else (None,)
+        variants = (None, "site", "tile_tma") if p == 32 else (None, "site")
         qk[f"f{p}_recon{r}"] = measure_q_kernel(torch, nd, gdims, args.lattice, U64, p, r, peak, variants)
     q_clocks = q_sampler.stop()
     main = qk[f"f{prec}_recon{recon}"]
@@ -676,6 +693,8 @@ def main():
     ap.add_argument("--eig-degree", type=int, default=100)
     ap.add_argument("--quick", action="store_true", help="headline + its own Q-kernel variant only (no layout / configs legs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--q-only", action="store_true", help="time only the Q stencil of --prec / --recon on --lattice (plain and fused epilogue)")
+    ap.add_argument("--variant", default=None, choices=["site", "tile", "tile_tma"], help="with --q-only: force a stencil variant")
     ap.add_argument("--replicas", action="store_true", help="--gpus N as N independent lattices (weak scaling) instead of the domain decomposition")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup

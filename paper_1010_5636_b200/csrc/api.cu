@@ -140,7 +140,9 @@ extern "C" int nd_set_stencil_variant(nd_ctx* ctx, int variant) {
     if (variant != ND_STENCIL_AUTO && variant != ND_STENCIL_SITE && variant != ND_STENCIL_TILE && variant != ND_STENCIL_TILE_TMA)
         return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: unknown variant %d", variant);
     if ((variant == ND_STENCIL_TILE || variant == ND_STENCIL_TILE_TMA) && !ctx->tile_ok)
-        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: the tiled kernel needs fp32, x3 extent 32, even x1 / x2 extents and >= 8 tiles per SM");
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: the tiled kernels need x3 extent 32, even x1 / x2 extents (fp64: >= 4, recon 12 / 8) and >= 8 tiles per SM");
+    if (variant == ND_STENCIL_TILE_TMA && ctx->prec != 32)
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: the TMA bulk-copy variant exists in fp32 only");
     ctx->stencil_variant = variant;
     ndi_drop_graphs(ctx);
     return ND_OK;

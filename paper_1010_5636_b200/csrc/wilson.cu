@@ -294,8 +294,6 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
     if (v1 == in || v2 == in || v3 == in) {
         // allowed (read-only), nothing to do
     }
-    // the tiled marching kernel (wilson_tile.cu) where it is the faster one: fp32 on lattices it supports; with the
-    // uncompressed recon-18 links (64-bit words in fp32) only the fused-epilogue variant wins (224 vs 199 us plain, 252 vs 276 us fused)
     if (ctx->shard_n > 1 && !ctx->in_shard_call) {
         // domain decomposition (shard.cu): faces out, the local stencil with the wrapped time hops switched off while the
         // transfer runs, faces in.  One right-hand side at a time (the halo buffers hold one face pair).
@@ -320,7 +318,10 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
         }
         return ND_OK;
     }
-    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->recon != 18 || epi))
+    // the tiled marching kernels (wilson_tile.cu) where they are the faster ones on 32^3x64 (us per launch, tile vs site):
+    //   fp32 recon 12 / 8: plain 145 vs 167, fused 224 vs 240; fp32 recon 18 (64-bit link words): fused only (252 vs 276; plain 224 vs 199)
+    //   fp64 recon 12 / 8: plain only (289 vs 344; the fused-epilogue stencil is at 87 % of the HBM peak in the site kernel: 502 vs 512)
+    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->prec == 32 ? (ctx->recon != 18 || epi) : !epi))
                                                                 : (ctx->stencil_variant != ND_STENCIL_SITE);
     if (tile) {   // large lattices: one launch per right-hand side already fills the machine
         const size_t sb = nd_spinor_bytes(ctx);

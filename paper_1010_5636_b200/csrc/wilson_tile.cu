@@ -44,6 +44,18 @@ __device__ __forceinline__ void words_to_half(const float4 (&w)[3], cx<float> (&
     h[0][2] = {w[1].x, w[1].y}; h[1][0] = {w[1].z, w[1].w};
     h[1][1] = {w[2].x, w[2].y}; h[1][2] = {w[2].z, w[2].w};
 }
+__device__ __forceinline__ void half_to_words(const cx<double> (&h)[2][3], double2 (&w)[6]) {
+#pragma unroll
+    for (int s = 0; s < 2; s++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) w[3 * s + c] = make_double2(h[s][c].re, h[s][c].im);
+}
+__device__ __forceinline__ void words_to_half(const double2 (&w)[6], cx<double> (&h)[2][3]) {
+#pragma unroll
+    for (int s = 0; s < 2; s++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) h[s][c] = {w[3 * s + c].x, w[3 * s + c].y};
+}
 // slot (kind, site) of one exchange buffer: words [kind][w][site], consecutive lanes on consecutive 128-bit words
 template <typename T, int NT>
 __device__ __forceinline__ void put_half(typename Prec<T>::Vec* buf, int kind, int site, const cx<T> (&h)[2][3]) {
@@ -63,6 +75,7 @@ __device__ __forceinline__ void get_half(const typename Prec<T>::Vec* buf, int k
 }
 
 __device__ __forceinline__ float shfl_real(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+__device__ __forceinline__ double shfl_real(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 template <typename T> __device__ __forceinline__ void shfl_half(cx<T> (&h)[2][3], int src) {
 #pragma unroll
     for (int s = 0; s < 2; s++)
@@ -133,10 +146,11 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
 
 // The halo slot of a tile-face thread: the spinor (and, for a backward face, the link) of its neighbour outside the tile,
 // fetched by cp.async one phase ahead: words [NV spinor planes][NT] then [NL link words][NT].
-template <typename T, int RECON, int MU, int NT>
+// (HLN entries per link word, entry `hidx` of this thread: the fp64 kernel keeps link entries for the backward faces only)
+template <typename T, int RECON, int MU, int NT, int HLN = NT>
 __device__ __forceinline__ void issue_halo(unsigned char* hal, const typename Prec<T>::Vec* __restrict__ in,
                                            const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, long long V, int site,
-                                           bool face_bwd, bool face_fwd, long long s_bwd, long long s_fwd) {
+                                           bool face_bwd, bool face_fwd, long long s_bwd, long long s_fwd, int hidx) {
     using Vec = typename Prec<T>::Vec;
     using LL = LinkLayout<T, RECON>;
     Vec* hs = reinterpret_cast<Vec*>(hal);
@@ -148,7 +162,7 @@ __device__ __forceinline__ void issue_halo(unsigned char* hal, const typename Pr
     }
     if (face_bwd) {
 #pragma unroll
-        for (int p = 0; p < LL::NL; p++) cp_async<sizeof(typename LL::LVec)>(&hl[p * NT + site], gauge + ((long long)MU * LL::NL + p) * V + s_bwd);
+        for (int p = 0; p < LL::NL; p++) cp_async<sizeof(typename LL::LVec)>(&hl[p * HLN + hidx], gauge + ((long long)MU * LL::NL + p) * V + s_bwd);
     }
 }
 
@@ -182,9 +196,10 @@ template <typename T, int RECON> __device__ __forceinline__ unsigned halo_bytes(
 // One direction mu in {1, 2} of the send phase of a site: the two half-spinors its in-tile neighbours need, and, on a tile
 // face, the half-spinor this site itself needs from outside the tile (neighbour data from the halo slot).
 //   slot kinds K = "h- of my forward neighbour" (read in the forward hop), K + 1 = "w of my backward neighbour"
-template <typename T, int RECON, int MU, int NT, int K>
+template <typename T, int RECON, int MU, int NT, int K, int HLN = NT>
 __device__ __forceinline__ void send_dir(typename Prec<T>::Vec* buf, const unsigned char* hal, const cx<T> (&phi)[12],
-                                         const cx<T> (&U)[3][3], int site, int slot_bwd, int slot_fwd, bool face_bwd, bool face_fwd) {
+                                         const cx<T> (&U)[3][3], int site, int slot_bwd, int slot_fwd, bool face_bwd, bool face_fwd,
+                                         int hidx) {
     using Vec = typename Prec<T>::Vec;
     using LL = LinkLayout<T, RECON>;
     cx<T> h[2][3], g[2][3];
@@ -211,7 +226,7 @@ __device__ __forceinline__ void send_dir(typename Prec<T>::Vec* buf, const unsig
             const typename LL::LVec* hl = reinterpret_cast<const typename LL::LVec*>(hal + (size_t)Prec<T>::NV * NT * sizeof(Vec));
             typename LL::LVec lw[LL::NL];
 #pragma unroll
-            for (int p = 0; p < LL::NL; p++) lw[p] = hl[p * NT + site];
+            for (int p = 0; p < LL::NL; p++) lw[p] = hl[p * HLN + hidx];
             cx<T> Ub[3][3];
             reconstruct_link<T, RECON>(lw, Ub);
             project<T, MU, +1>(psi, T(1), h);
@@ -408,7 +423,7 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
         issue_halo_bulk<T, RECON, 1, NT>(hal, in, gauge, G.V, row0, lane, face_b1, face_f1, ts * G.S0 + ss_b1 - lane, ts * G.S0 + ss_f1 - lane, bar_top);
         if (lane == 0) mbar_expect_tx(bar_top, top_bytes);
     } else {
-        issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, ts * G.S0 + ss_b1, ts * G.S0 + ss_f1);
+        issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, ts * G.S0 + ss_b1, ts * G.S0 + ss_f1, site);
         cp_async_commit();
     }
 
@@ -454,14 +469,14 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
             if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 1, site, lane, more, s_next - lane, bar_top, U);
             else take_link<T, RECON, NT>(lnk, gauge, G.V, 1, site, more, s_next, U);
             kept.keep(U);
-            send_dir<T, RECON, 1, NT, 0>(xbuf, hal, phi_c, U, site, slot_b1, slot_f1, face_b1, face_f1);
+            send_dir<T, RECON, 1, NT, 0>(xbuf, hal, phi_c, U, site, slot_b1, slot_f1, face_b1, face_f1, site);
             // the halo slot is free again: this slice's x2 halo
             if (BULK) {
                 __syncwarp();
                 issue_halo_bulk<T, RECON, 2, NT>(hal, in, gauge, G.V, row0, lane, face_b2, face_f2, st + ss_b2 - lane, st + ss_f2 - lane, bar_mid);
                 if (lane == 0) mbar_expect_tx(bar_mid, halo_bytes<T, RECON>(face_b2, face_f2));
             } else {
-                issue_halo<T, RECON, 2, NT>(hal, in, gauge, G.V, site, face_b2, face_f2, st + ss_b2, st + ss_f2);
+                issue_halo<T, RECON, 2, NT>(hal, in, gauge, G.V, site, face_b2, face_f2, st + ss_b2, st + ss_f2, site);
                 cp_async_commit();
             }
         }
@@ -496,14 +511,14 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
             // the x2 halo
             if (BULK) mbar_wait(bar_mid, i & 1);
             else cp_async_wait_all();
-            send_dir<T, RECON, 2, NT, K2>(xbuf, hal, phi_c, U, site, slot_b2, slot_f2, face_b2, face_f2);
+            send_dir<T, RECON, 2, NT, K2>(xbuf, hal, phi_c, U, site, slot_b2, slot_f2, face_b2, face_f2, site);
             if (more) {
                 if (BULK) {
                     __syncwarp();
                     issue_halo_bulk<T, RECON, 1, NT>(hal, in, gauge, G.V, row0, lane, face_b1, face_f1, st + G.S0 + ss_b1 - lane,
                                                      st + G.S0 + ss_f1 - lane, bar_top);
                 } else {
-                    issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, st + G.S0 + ss_b1, st + G.S0 + ss_f1);
+                    issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, st + G.S0 + ss_b1, st + G.S0 + ss_f1, site);
                 }
             }
         }
@@ -549,6 +564,249 @@ int choose_segments(int L0, int ntile, int slots) {
         if (eff > best_eff + 1e-9) { best_eff = eff; best = nseg; }
     }
     return best;
+}
+
+// ------------------------------------------------------------------------------------------ the fp64 variant
+// In fp64 a site's state is twice as large, and the kernel above neither fits the register file (next spinor of the column
+// and a whole kept link on top of accumulators, current spinor and carried time hop: 255 registers and spills) nor shared
+// memory (135 KB per 128 sites: one CTA of 4 warps per SM).  Same march, same exchange, different staging:
+//   * the NEXT spinor of the column is not held in registers: it travels by cp.async into a private slot and is read at the
+//     forward time hop, into the registers of the current spinor, which is dead by then;
+//   * TWO link slots instead of four, each shared by two directions in turn (A: x1, then x2; B: x3, then x0): a slot is
+//     refilled as soon as its link has been read, so a link is in flight for about half a time-slice (2 CTAs per SM alternate:
+//     a few microseconds) instead of a whole one;
+//   * the halo slot keeps link entries only for the three rows of the tile that have a backward face;
+//   * cp.async groups are committed at four points of a slice and every wait is "all but the newest group".
+// Shared memory (recon 12): 24 (exchange) + 24 (links) + 24 + 9 (halo) + 24 (next spinor) = 105 KB: two CTAs per SM.
+// Tile 2 x 2 x 32 with the pair barriers of the kernel above; x1 and x2 extents of at least 4 (every site of the tile has
+// exactly one neighbour outside the tile per direction).
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <typename T, int RECON, int NT>
+__device__ __forceinline__ void read_link_slot(const typename LinkLayout<T, RECON>::LVec* slot, int site, cx<T> (&U)[3][3]) {
+    using LL = LinkLayout<T, RECON>;
+    typename LL::LVec w[LL::NL];
+#pragma unroll
+    for (int p = 0; p < LL::NL; p++) w[p] = slot[p * NT + site];
+    reconstruct_link<T, RECON>(w, U);
+}
+template <typename T, int RECON, int NT>
+__device__ __forceinline__ void fill_link_slot(typename LinkLayout<T, RECON>::LVec* slot, const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge,
+                                               long long V, int mu, int site, long long s) {
+    using LL = LinkLayout<T, RECON>;
+    const typename LL::LVec* src = gauge + (long long)mu * LL::NL * V + s;
+#pragma unroll
+    for (int p = 0; p < LL::NL; p++) cp_async<sizeof(typename LL::LVec)>(&slot[p * NT + site], src + p * V);
+}
+
+template <typename T, int RECON, bool EPI, int MINB>
+__global__ void __launch_bounds__(128, MINB)
+    wilson_Q_tile2_kernel(typename Prec<T>::Vec* out, const typename Prec<T>::Vec* __restrict__ in,
+                          const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, TileGeom G, T mass_term, T s0, T s1,
+                          const typename Prec<T>::Vec* v1, T s2, const typename Prec<T>::Vec* v2, T s3,
+                          const typename Prec<T>::Vec* v3) {
+    using Vec = typename Prec<T>::Vec;
+    using LL = LinkLayout<T, RECON>;
+    using LVec = typename LL::LVec;
+    constexpr int B2 = 2, L3 = 32, NT = 128, HLN = 3 * L3;   // halo link entries: the three rows with a backward face
+    constexpr int NW = HalfWords<T>::NW, NV = Prec<T>::NV;
+    constexpr int ROW1 = B2 * L3, ROW2 = L3;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    unsigned char* sp = smem_raw;
+    Vec* xbuf = reinterpret_cast<Vec*>(sp);   sp += (size_t)2 * NW * NT * sizeof(Vec);        // exchange: [2 kinds][NW][NT]
+    LVec* lnkA = reinterpret_cast<LVec*>(sp); sp += (size_t)LL::NL * NT * sizeof(LVec);       // link slot A: x1, then x2
+    LVec* lnkB = reinterpret_cast<LVec*>(sp); sp += (size_t)LL::NL * NT * sizeof(LVec);       // link slot B: x3, then x0
+    unsigned char* hal = sp;                  sp += (size_t)NV * NT * sizeof(Vec) + (size_t)LL::NL * HLN * sizeof(LVec);   // halo slot
+    Vec* phis = reinterpret_cast<Vec*>(sp);                                                    // next spinor of the column: [NV][NT]
+
+    const int site = threadIdx.x;
+    const int x3 = site % L3, r2 = (site / L3) % B2, r1 = site / (L3 * B2);
+    const int tile = blockIdx.x % G.ntile, seg = blockIdx.x / G.ntile;
+    const int x1 = (tile / G.nt2) * 2 + r1, x2 = (tile % G.nt2) * 2 + r2;
+    const long long S1 = (long long)G.L2 * L3, S2 = L3;
+    const long long ss = ((long long)x1 * G.L2 + x2) * L3 + x3;
+    const int ts = seg * G.seg_base + (seg < G.seg_rem ? seg : G.seg_rem);
+    const int len = G.seg_base + (seg < G.seg_rem ? 1 : 0);
+    const int lane = threadIdx.x & 31;
+
+    // in-tile neighbours (the other row of the pair) and the neighbours outside the tile
+    const bool face_b1 = (r1 == 0), face_f1 = !face_b1, face_b2 = (r2 == 0), face_f2 = !face_b2;
+    const int slot_b1 = face_b1 ? -1 : site - ROW1, slot_f1 = face_f1 ? -1 : site + ROW1;
+    const int slot_b2 = face_b2 ? -1 : site - ROW2, slot_f2 = face_f2 ? -1 : site + ROW2;
+    const long long ss_b1 = (x1 == 0) ? ss + (long long)(G.L1 - 1) * S1 : ss - S1;
+    const long long ss_f1 = (x1 == G.L1 - 1) ? ss - (long long)(G.L1 - 1) * S1 : ss + S1;
+    const long long ss_b2 = (x2 == 0) ? ss + (long long)(G.L2 - 1) * S2 : ss - S2;
+    const long long ss_f2 = (x2 == G.L2 - 1) ? ss - (long long)(G.L2 - 1) * S2 : ss + S2;
+    // halo link entry of this thread, the same in both directions (private: no other thread ever touches it): rows
+    // (r1, r2) = (0, 0) [backward face in x1 and x2], (0, 1) [x1 only], (1, 0) [x2 only]
+    const int hidx1 = x3 + L3 * (r1 == 0 ? r2 : 2), hidx2 = hidx1;
+    const int lane_f3 = (lane + 1) & (L3 - 1), lane_b3 = (lane + L3 - 1) & (L3 - 1);
+
+    // group a: link 1 and the x1 halo of the first slice; group b: link 3 of the first slice and the spinor of the second
+    fill_link_slot<T, RECON, NT>(lnkA, gauge, G.V, 1, site, ts * G.S0 + ss);
+    issue_halo<T, RECON, 1, NT, HLN>(hal, in, gauge, G.V, site, face_b1, face_f1, ts * G.S0 + ss_b1, ts * G.S0 + ss_f1, hidx1);
+    cp_async_commit();
+    fill_link_slot<T, RECON, NT>(lnkB, gauge, G.V, 3, site, ts * G.S0 + ss);
+    {
+        const long long sn = ((ts == G.L0 - 1) ? 0 : (ts + 1) * G.S0) + ss;
+#pragma unroll
+        for (int p = 0; p < NV; p++) cp_async<16>(&phis[p * NT + site], in + p * G.V + sn);
+    }
+    cp_async_commit();
+
+    cx<T> phi_c[12], w0[2][3];
+    {
+        // the backward time hop of the segment's first slice: U_0(x, t-1)^dagger (1 + gamma_0) phi(x, t-1)
+        const int tp = (ts == 0) ? G.L0 - 1 : ts - 1;
+        cx<T> psi[12], U[3][3], h[2][3];
+        load_spinor<T>(in, G.V, tp * G.S0 + ss, psi);
+        load_link<T, RECON>(gauge, G.V, 0, tp * G.S0 + ss, U);
+        project<T, 0, +1>(psi, (ts == 0) ? T(G.bc) : T(1), h);
+        mul_Udag(U, h, w0);
+        load_spinor<T>(in, G.V, ts * G.S0 + ss, phi_c);
+    }
+
+    for (int i = 0; i < len; i++) {
+        const int t = ts + i;
+        const long long st = t * G.S0;
+        const long long s = st + ss;
+        const bool more = (i + 1 < len);
+        cp_async_wait<1>();                        // link 1 and the x1 halo of this slice have landed
+        if (EPI && (lane & 7) == 0) {
+            // the fused update's vectors of this slice are read after the last barrier, with no registers to load them early:
+            // pull their lines (8 lanes = one 128-byte line per plane) into L2 now, a whole slice ahead
+            const Vec* vs[3] = {v1, v2, v3};
+#pragma unroll
+            for (int j = 0; j < 3; j++)
+                if (vs[j]) {
+#pragma unroll
+                    for (int p = 0; p < NV; p++) asm volatile("prefetch.global.L2 [%0];" ::"l"(vs[j] + p * G.V + s));
+                }
+        }
+        cx<T> acc[12];
+        {
+            const T f = T(-2) * mass_term;
+#pragma unroll
+            for (int k = 0; k < 12; k++) acc[k] = {f * phi_c[k].re, f * phi_c[k].im};
+        }
+        KeptLink<T> kept;
+        // ---- x1: send
+        pair_barrier(1 + r2);
+        {
+            cx<T> U[3][3];
+            read_link_slot<T, RECON, NT>(lnkA, site, U);
+            fill_link_slot<T, RECON, NT>(lnkA, gauge, G.V, 2, site, s);             // slot A: link 2 of this slice
+            kept.keep(U);
+            send_dir<T, RECON, 1, NT, 0, HLN>(xbuf, hal, phi_c, U, site, slot_b1, slot_f1, face_b1, face_f1, hidx1);
+            issue_halo<T, RECON, 2, NT, HLN>(hal, in, gauge, G.V, site, face_b2, face_f2, st + ss_b2, st + ss_f2, hidx2);
+            cp_async_commit();                     // group 1
+        }
+        // ---- x3: lanes of this warp
+        cp_async_wait<1>();                        // link 3 (and the next spinor of the column)
+        {
+            cx<T> U[3][3], h[2][3], g[2][3];
+            read_link_slot<T, RECON, NT>(lnkB, site, U);
+            fill_link_slot<T, RECON, NT>(lnkB, gauge, G.V, 0, site, s);             // slot B: link 0 of this slice
+            cp_async_commit();                     // group 2
+            project<T, 3, -1>(phi_c, T(1), h);
+            shfl_half(h, lane_f3);
+            mul_U(U, h, g);
+            accumulate<T, 3, -1>(g, acc);
+            project<T, 3, +1>(phi_c, T(1), h);
+            mul_Udag(U, h, g);
+            shfl_half(g, lane_b3);
+            accumulate<T, 3, +1>(g, acc);
+        }
+        pair_barrier(1 + r2);                      // x1 half-spinors are in place
+        {
+            cx<T> U[3][3];
+            kept.get(U);
+            recv_dir<T, 1, NT, 0>(xbuf, U, site, acc);
+        }
+        // ---- x2: send
+        pair_barrier(3 + r1);
+        cp_async_wait<1>();                        // link 2 and the x2 halo
+        {
+            cx<T> U[3][3];
+            read_link_slot<T, RECON, NT>(lnkA, site, U);
+            if (more) fill_link_slot<T, RECON, NT>(lnkA, gauge, G.V, 1, site, s + G.S0);   // slot A: link 1 of the next slice
+            kept.keep(U);
+            send_dir<T, RECON, 2, NT, 0, HLN>(xbuf, hal, phi_c, U, site, slot_b2, slot_f2, face_b2, face_f2, hidx2);
+            if (more) issue_halo<T, RECON, 1, NT, HLN>(hal, in, gauge, G.V, site, face_b1, face_f1, st + G.S0 + ss_b1, st + G.S0 + ss_f1, hidx1);
+            cp_async_commit();                     // group 3
+        }
+        // ---- x0: this thread's own column
+        cp_async_wait<1>();                        // link 0
+        {
+            cx<T> U[3][3], h[2][3], g[2][3];
+            const T ph = (t == G.L0 - 1) ? T(G.bc) : T(1);
+            accumulate<T, 0, +1>(w0, acc);         // carried from the previous slice
+            read_link_slot<T, RECON, NT>(lnkB, site, U);
+            if (more) fill_link_slot<T, RECON, NT>(lnkB, gauge, G.V, 3, site, s + G.S0);   // slot B: link 3 of the next slice
+            project<T, 0, +1>(phi_c, ph, h);
+            mul_Udag(U, h, w0);                    // the next slice's backward time hop; phi(t) is dead now
+            {
+                Vec w[NV];
+#pragma unroll
+                for (int p = 0; p < NV; p++) w[p] = phis[p * NT + site];
+                words_to_cx(w, phi_c);             // phi(t + 1)
+            }
+            if (more) {                            // the slot takes phi(t + 2) (exists: t + 1 <= L0 - 1)
+                const long long sn = ((t + 1 == G.L0 - 1) ? 0 : st + 2 * G.S0) + ss;
+#pragma unroll
+                for (int p = 0; p < NV; p++) cp_async<16>(&phis[p * NT + site], in + p * G.V + sn);
+            }
+            cp_async_commit();                     // group 4
+            project<T, 0, -1>(phi_c, ph, h);
+            mul_U(U, h, g);
+            accumulate<T, 0, -1>(g, acc);
+        }
+        EpiVectors<T, EPI> ev;
+        ev.load(G.V, s, s1, v1, s2, v2, s3, v3);
+        pair_barrier(3 + r1);                      // x2 half-spinors are in place
+        {
+            cx<T> U[3][3];
+            kept.get(U);
+            recv_dir<T, 2, NT, 0>(xbuf, U, site, acc);
+        }
+        ev.finish(out, G.V, s, acc, s0, s1, s2, s3);
+    }
+}
+
+template <typename T, int RECON, bool EPI, int MINB>
+int launch_tile2(nd_ctx* ctx, void* out, const void* in, double m, double s0, double s1, const void* v1, double s2, const void* v2,
+                 double s3, const void* v3) {
+    using Vec = typename Prec<T>::Vec;
+    using LL = LinkLayout<T, RECON>;
+    using LVec = typename LL::LVec;
+    constexpr int NT = 128;
+    constexpr size_t smem = (size_t)2 * HalfWords<T>::NW * NT * sizeof(Vec) + (size_t)2 * LL::NL * NT * sizeof(LVec) +
+                            (size_t)Prec<T>::NV * NT * sizeof(Vec) + (size_t)LL::NL * 96 * sizeof(LVec) +
+                            (size_t)Prec<T>::NV * NT * sizeof(Vec);
+    TileGeom G;
+    G.L0 = ctx->dims[0]; G.L1 = ctx->dims[1]; G.L2 = ctx->dims[2];
+    G.V = ctx->V;
+    G.S0 = (long long)ctx->dims[1] * ctx->dims[2] * ctx->dims[3];
+    G.bc = ctx->bc;
+    G.nt2 = G.L2 / 2;
+    G.ntile = (G.L1 / 2) * G.nt2;
+    auto kern = wilson_Q_tile2_kernel<T, RECON, EPI, MINB>;
+    int& per_sm = ctx->tile_ctas_per_sm[EPI ? 1 : 0];
+    if (per_sm == 0) {
+        ND_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int n = 0;
+        ND_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, NT, smem));
+        if (n < 1) return nd_fail(ctx, ND_ERR_CUDA, "tiled fp64 stencil does not fit on an SM");
+        per_sm = n;
+    }
+    const int nseg = choose_segments(G.L0, G.ntile, per_sm * ctx->num_sms);
+    G.seg_base = G.L0 / nseg;
+    G.seg_rem = G.L0 % nseg;
+    const unsigned blocks = (unsigned)(G.ntile * nseg);
+    kern<<<blocks, NT, smem, ctx->stream>>>((Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(s0), T(s1),
+                                            (const Vec*)v1, T(s2), (const Vec*)v2, T(s3), (const Vec*)v3);
+    ND_LAUNCHED(ctx);
+    return ND_OK;
 }
 
 template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB, bool BULK>
@@ -605,21 +863,29 @@ int launch_tile_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi
 
 }  // namespace
 
-// Lattices the tiled kernel takes: fp32 (in fp64 a site's state - accumulators, the current and the next spinor of the column,
-// the carried time hop, a kept link - does not fit the register file at a useful occupancy: measured 357 / 600 us per launch
-// on 32^3x64 against 349 / 498 us of the site-per-thread kernel), x3 extent 32 (tile 2 x 2 x 32) or
-// 16 (tile 2 x 4 x 16), even x1 / x2 extents divisible by the tile, and enough tiles to give every SM work.
+// Lattices the tiled kernels take: x3 extent 32 (tile 2 x 2 x 32: a warp is one x3 row), even x1 / x2 extents, and enough tiles
+// to give every SM work.  fp32: wilson_Q_tile_kernel; fp64: wilson_Q_tile2_kernel (x1, x2 extents >= 4, recon 12 / 8).
 bool ndi_tile_supported(const nd_ctx* ctx) {
     const int L1 = ctx->dims[1], L2 = ctx->dims[2], L3 = ctx->dims[3];
-    if (ctx->prec != 32) return false;
-    const int b1 = 2, b2 = 2;
     if (L3 != 32) return false;
-    if (L1 % b1 != 0 || L2 % b2 != 0) return false;
-    return (long long)(L1 / b1) * (L2 / b2) * ctx->dims[0] >= 8LL * ctx->num_sms;
+    if (L1 % 2 != 0 || L2 % 2 != 0) return false;
+    if (ctx->prec == 64 && (L1 < 4 || L2 < 4 || ctx->recon == 18)) return false;
+    return (long long)(L1 / 2) * (L2 / 2) * ctx->dims[0] >= 8LL * ctx->num_sms;
+}
+
+template <int RECON>
+static int launch_tile2_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
+                       const void* v2, double s3, const void* v3) {
+    if (epi) return launch_tile2<double, RECON, true, 2>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile2<double, RECON, false, 2>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
 }
 
 int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                      const void* v2, double s3, const void* v3) {
+    if (ctx->prec == 64) {
+        if (ctx->recon == 12) return launch_tile2_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile2_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    }
     if (ctx->recon == 18) return launch_tile_shape<18>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);   // (fused epilogue only)
     if (ctx->recon == 12) return launch_tile_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
     return launch_tile_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);

@@ -44,6 +44,38 @@ def test_every_variant_matches_the_oracle(dims, bc, recon):
     assert np.abs(results["tile"] - ref).max() <= (2e-5 if recon != 8 else 2e-4) * scale
 
 
+@pytest.mark.parametrize("dims,bc", [((40, 8, 16, 32), -1), ((152, 4, 16, 32), -1), ((80, 16, 4, 32), +1)])
+@pytest.mark.parametrize("recon", [12, 8])
+def test_fp64_tiled_kernel_matches_the_oracle(dims, bc, recon):
+    """wilson_Q_tile2_kernel (two link slots, next spinor through shared memory): segments, the seam, boundary tiles, x1 / x2
+    extent 4 (both outside neighbours of a pair are the same row of the neighbouring tile)."""
+    ctx, U = make_context(dims, 64, recon, bc, "smooth", eps=0.3)
+    psi = gaussian_spinor(dims)
+    vecs = [gaussian_spinor(dims, seed=20 + i) for i in range(3)]
+    x, y = ctx.pack_spinor(psi), ctx.new_spinor()
+    d = [ctx.pack_spinor(v) for v in vecs]
+    ref = wilson_c.apply_Q(psi, U, -1.6, bc)
+    s0, s1, s2, s3 = 0.37, -1.2, -1.0, 0.81
+    ref_epi = s0 * ref + s1 * vecs[0] + s2 * vecs[1] + s3 * vecs[2]
+    results, fused = {}, {}
+    for variant in ("site", "tile", "auto"):
+        ctx.set_stencil_variant(variant)
+        assert ctx.get_stencil_variant() == ("tile" if variant == "auto" else variant)
+        ctx.apply_Q(y, x, -1.6)
+        got = ctx.unpack_spinor(y)
+        assert rel_l2(got, ref) <= TOL[64], (variant, rel_l2(got, ref))
+        results[variant] = got
+        out = ctx.new_spinor()
+        ctx.copy(out, d[1])
+        ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])
+        fused[variant] = ctx.unpack_spinor(out)
+        assert rel_l2(fused[variant], ref_epi) <= TOL[64], variant
+    # auto in fp64: the tiled kernel for the plain stencil, the site-per-thread kernel for the fused-epilogue one
+    assert np.array_equal(results["auto"], results["tile"]) and np.array_equal(fused["auto"], fused["site"])
+    scale = np.abs(ref).max()
+    assert np.abs(results["tile"] - ref).max() <= (1e-13 if recon != 8 else 1e-10) * scale
+
+
 def test_variant_selection_rules():
     import paper_1010_5636_b200 as nd
 
@@ -52,7 +84,10 @@ def test_variant_selection_rules():
     with pytest.raises(nd.NDError) as e:
         ctx.set_stencil_variant("tile")
     assert e.value.code == -1
-    ctx64, _ = make_context((40, 8, 16, 32), 64, 12)                 # fp64: site-per-thread kernel
-    assert ctx64.get_stencil_variant() == "site"
+    ctx64, _ = make_context((40, 8, 16, 32), 64, 12)
+    assert ctx64.get_stencil_variant() == "tile"
     with pytest.raises(nd.NDError):
-        ctx64.set_stencil_variant("tile_tma")
+        ctx64.set_stencil_variant("tile_tma")                        # the bulk-copy variant exists in fp32 only
+    ctx64b, _ = make_context((40, 2, 16, 32), 64, 12)                # fp64 tiles need x1 / x2 extents >= 4
+    with pytest.raises(nd.NDError):
+        ctx64b.set_stencil_variant("tile")
