@@ -71,14 +71,15 @@ ND_API long long nd_volume(const nd_ctx* ctx);          /* number of sites V */
 ND_API size_t nd_spinor_bytes(const nd_ctx* ctx);       /* bytes of one device SoA spinor = 24 * V * prec/8 */
 ND_API size_t nd_gauge_bytes(const nd_ctx* ctx);        /* bytes of the compressed device gauge field */
 /* Which kernel applies the stencil (csrc/wilson.cu, csrc/wilson_tile.cu).  ND_STENCIL_AUTO (default)
- * picks the fastest one measured for the context and call: the tiled marching kernels (neighbour exchange through shared memory,
- * cp.async prefetch) on lattices they support - x3 extent 32, even x1 / x2 extents (fp64: >= 4, recon 12 / 8), at least 8 tiles
- * per SM; in fp64 for the plain stencil only - and the site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The
- * other values force one kernel for every call, for parity tests and for timing the variants against each other
- * (ND_STENCIL_TILE_TMA: the fp32 tiled kernel with TMA bulk copies instead of cp.async); ND_ERR_BAD_ARG if the context cannot
- * run it.  Cached CUDA graphs are dropped.  nd_get_stencil_variant returns the variant in effect for the plain stencil (never
- * ND_STENCIL_AUTO). */
-enum { ND_STENCIL_AUTO = 0, ND_STENCIL_SITE = 1, ND_STENCIL_TILE = 2, ND_STENCIL_TILE_TMA = 3 };
+ * picks the fastest one measured for the context and call: the tiled marching kernel (neighbour exchange through shared memory,
+ * cp.async prefetch of links, halos and the next spinor) on lattices it supports - x3 extent 32 or 16, even x1 / x2 extents >= 4
+ * (x3 extent 16: x2 extent divisible by 4), at least 8 slices of 128 sites per SM, in fp64 recon 12 / 8 and the plain stencil
+ * only - and the site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The other values force one kernel for every call, for parity tests and for timing the variants against
+ * each other: ND_STENCIL_SITE, ND_STENCIL_TILE (the tiled kernel above), and in fp32 its predecessor with four link slots and
+ * the next spinor in registers (x3 extent 32), prefetching by cp.async (ND_STENCIL_TILE4) or by TMA bulk copies (ND_STENCIL_TILE_TMA);
+ * ND_ERR_BAD_ARG if the context cannot run it.  Cached CUDA graphs are dropped.  nd_get_stencil_variant returns the variant in
+ * effect for the plain stencil (never ND_STENCIL_AUTO). */
+enum { ND_STENCIL_AUTO = 0, ND_STENCIL_SITE = 1, ND_STENCIL_TILE = 2, ND_STENCIL_TILE_TMA = 3, ND_STENCIL_TILE4 = 4 };
 ND_API int nd_set_stencil_variant(nd_ctx* ctx, int variant);
 ND_API int nd_get_stencil_variant(const nd_ctx* ctx);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */

@@ -309,7 +309,7 @@ class Context:
         raw.__cuda_array_interface__ = {"shape": (nbytes // itemsize,), "typestr": typestr, "data": (int(ptr), False), "version": 2}
         return torch.as_tensor(raw, device=self.torch_device)
 
-    STENCIL = {"auto": 0, "site": 1, "tile": 2, "tile_tma": 3}
+    STENCIL = {"auto": 0, "site": 1, "tile": 2, "tile_tma": 3, "tile4": 4}
 
     def set_stencil_variant(self, name):
         self._chk(self.lib.nd_set_stencil_variant(self._h, self.STENCIL[name]))

@@ -219,11 +219,27 @@ __global__ void __launch_bounds__(LAYOUT_THREADS) compress_gauge_kernel(typename
         rerr = fmax(rerr, __shfl_xor_sync(0xffffffffu, rerr, o));
         N = fmin(N, __shfl_xor_sync(0xffffffffu, N, o));
     }
+    // ... one CTA-level reduction through shared memory, and an atomic only where the CTA improves on the value already there
+    // (tens of thousands of CTAs hammering four addresses with atomics were the kernel's bottleneck)
+    __shared__ double cta_stats[LAYOUT_THREADS / 32][4];
     if ((threadIdx.x & 31) == 0) {
-        atomic_max_nonneg(stats + 0, dev);
-        atomic_max_nonneg(stats + 1, ddev);
-        atomic_min_nonneg(stats + 2, N);
-        atomic_max_nonneg(stats + 3, rerr);
+        double* r = cta_stats[threadIdx.x >> 5];
+        r[0] = dev; r[1] = ddev; r[2] = N; r[3] = rerr;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int w = 1; w < LAYOUT_THREADS / 32; w++) {
+            dev = fmax(dev, cta_stats[w][0]);
+            ddev = fmax(ddev, cta_stats[w][1]);
+            N = fmin(N, cta_stats[w][2]);
+            rerr = fmax(rerr, cta_stats[w][3]);
+        }
+        const volatile double* cur = stats;
+        if (dev > cur[0]) atomic_max_nonneg(stats + 0, dev);
+        if (ddev > cur[1]) atomic_max_nonneg(stats + 1, ddev);
+        if (N < cur[2]) atomic_min_nonneg(stats + 2, N);
+        if (rerr > cur[3]) atomic_max_nonneg(stats + 3, rerr);
     }
     if (!valid) return;
     LVec* dst = g + (long long)mu * LL::NL * V + s0 + t;

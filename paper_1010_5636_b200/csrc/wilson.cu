@@ -318,10 +318,10 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
         }
         return ND_OK;
     }
-    // the tiled marching kernels (wilson_tile.cu) where they are the faster ones on 32^3x64 (us per launch, tile vs site):
-    //   fp32 recon 12 / 8: plain 145 vs 167, fused 224 vs 240; fp32 recon 18 (64-bit link words): fused only (252 vs 276; plain 224 vs 199)
-    //   fp64 recon 12 / 8: plain only (289 vs 344; the fused-epilogue stencil is at 87 % of the HBM peak in the site kernel: 502 vs 512)
-    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->prec == 32 ? (ctx->recon != 18 || epi) : !epi))
+    // the tiled marching kernel (wilson_tile.cu) where it is the faster one on 32^3x64 (us per launch, tile vs site):
+    //   fp32 recon 12 / 8 / 18: plain 139 / 148 / 171 vs 167 / 185 / 196, fused epilogue 224 / 226 / 252 vs 247 / 239 / 279
+    //   fp64 recon 12 / 8: plain 289 / 382 vs 344 / 417; fused 491 / 539 vs 502 / 535 (both at 87-89 % of the HBM peak): plain only
+    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->prec == 32 || !epi))
                                                                 : (ctx->stencil_variant != ND_STENCIL_SITE);
     if (tile) {   // large lattices: one launch per right-hand side already fills the machine
         const size_t sb = nd_spinor_bytes(ctx);

@@ -599,7 +599,7 @@ __device__ __forceinline__ void fill_link_slot(typename LinkLayout<T, RECON>::LV
     for (int p = 0; p < LL::NL; p++) cp_async<sizeof(typename LL::LVec)>(&slot[p * NT + site], src + p * V);
 }
 
-template <typename T, int RECON, bool EPI, int MINB>
+template <typename T, int RECON, bool EPI, int MINB, int L3>
 __global__ void __launch_bounds__(128, MINB)
     wilson_Q_tile2_kernel(typename Prec<T>::Vec* out, const typename Prec<T>::Vec* __restrict__ in,
                           const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, TileGeom G, T mass_term, T s0, T s1,
@@ -608,9 +608,12 @@ __global__ void __launch_bounds__(128, MINB)
     using Vec = typename Prec<T>::Vec;
     using LL = LinkLayout<T, RECON>;
     using LVec = typename LL::LVec;
-    constexpr int B2 = 2, L3 = 32, NT = 128, HLN = 3 * L3;   // halo link entries: the three rows with a backward face
+    // x3 extent 32: one 2 x 2 x 32 tile per CTA, a warp is one x3 row; x3 extent 16: two independent 2 x 2 x 16 tiles per CTA
+    // (neighbours in x2), a warp is the two rows (r2 = 0, 1) of one r1: the x2 partner of a site is in its own warp
+    constexpr int NT = 128, NSUB = 32 / L3, SUBT = NT / NSUB;
+    constexpr int HLN = 3 * 32;                // halo link entries: the three rows of a tile that have a backward face
     constexpr int NW = HalfWords<T>::NW, NV = Prec<T>::NV;
-    constexpr int ROW1 = B2 * L3, ROW2 = L3;
+    constexpr int ROW1 = 2 * L3, ROW2 = L3;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     unsigned char* sp = smem_raw;
     Vec* xbuf = reinterpret_cast<Vec*>(sp);   sp += (size_t)2 * NW * NT * sizeof(Vec);        // exchange: [2 kinds][NW][NT]
@@ -620,9 +623,9 @@ __global__ void __launch_bounds__(128, MINB)
     Vec* phis = reinterpret_cast<Vec*>(sp);                                                    // next spinor of the column: [NV][NT]
 
     const int site = threadIdx.x;
-    const int x3 = site % L3, r2 = (site / L3) % B2, r1 = site / (L3 * B2);
+    const int sub = site / SUBT, x3 = site % L3, r2 = (site / L3) % 2, r1 = (site / (2 * L3)) % 2;
     const int tile = blockIdx.x % G.ntile, seg = blockIdx.x / G.ntile;
-    const int x1 = (tile / G.nt2) * 2 + r1, x2 = (tile % G.nt2) * 2 + r2;
+    const int x1 = (tile / G.nt2) * 2 + r1, x2 = ((tile % G.nt2) * NSUB + sub) * 2 + r2;
     const long long S1 = (long long)G.L2 * L3, S2 = L3;
     const long long ss = ((long long)x1 * G.L2 + x2) * L3 + x3;
     const int ts = seg * G.seg_base + (seg < G.seg_rem ? seg : G.seg_rem);
@@ -639,8 +642,9 @@ __global__ void __launch_bounds__(128, MINB)
     const long long ss_f2 = (x2 == G.L2 - 1) ? ss - (long long)(G.L2 - 1) * S2 : ss + S2;
     // halo link entry of this thread, the same in both directions (private: no other thread ever touches it): rows
     // (r1, r2) = (0, 0) [backward face in x1 and x2], (0, 1) [x1 only], (1, 0) [x2 only]
-    const int hidx1 = x3 + L3 * (r1 == 0 ? r2 : 2), hidx2 = hidx1;
-    const int lane_f3 = (lane + 1) & (L3 - 1), lane_b3 = (lane + L3 - 1) & (L3 - 1);
+    const int hidx1 = sub * 3 * L3 + x3 + L3 * (r1 == 0 ? r2 : 2), hidx2 = hidx1;
+    const int lane_f3 = (lane & ~(L3 - 1)) | ((lane + 1) & (L3 - 1)), lane_b3 = (lane & ~(L3 - 1)) | ((lane + L3 - 1) & (L3 - 1));
+    const int bar1 = (L3 == 32) ? 1 + r2 : 1 + sub;   // the two warps that are x1 partners
 
     // group a: link 1 and the x1 halo of the first slice; group b: link 3 of the first slice and the spinor of the second
     fill_link_slot<T, RECON, NT>(lnkA, gauge, G.V, 1, site, ts * G.S0 + ss);
@@ -691,7 +695,7 @@ __global__ void __launch_bounds__(128, MINB)
         }
         KeptLink<T> kept;
         // ---- x1: send
-        pair_barrier(1 + r2);
+        pair_barrier(bar1);
         {
             cx<T> U[3][3];
             read_link_slot<T, RECON, NT>(lnkA, site, U);
@@ -717,14 +721,14 @@ __global__ void __launch_bounds__(128, MINB)
             shfl_half(g, lane_b3);
             accumulate<T, 3, +1>(g, acc);
         }
-        pair_barrier(1 + r2);                      // x1 half-spinors are in place
+        pair_barrier(bar1);                      // x1 half-spinors are in place
         {
             cx<T> U[3][3];
             kept.get(U);
             recv_dir<T, 1, NT, 0>(xbuf, U, site, acc);
         }
         // ---- x2: send
-        pair_barrier(3 + r1);
+        if (L3 == 32) pair_barrier(3 + r1); else __syncwarp();
         cp_async_wait<1>();                        // link 2 and the x2 halo
         {
             cx<T> U[3][3];
@@ -763,7 +767,7 @@ __global__ void __launch_bounds__(128, MINB)
         }
         EpiVectors<T, EPI> ev;
         ev.load(G.V, s, s1, v1, s2, v2, s3, v3);
-        pair_barrier(3 + r1);                      // x2 half-spinors are in place
+        if (L3 == 32) pair_barrier(3 + r1); else __syncwarp();                      // x2 half-spinors are in place
         {
             cx<T> U[3][3];
             kept.get(U);
@@ -773,7 +777,7 @@ __global__ void __launch_bounds__(128, MINB)
     }
 }
 
-template <typename T, int RECON, bool EPI, int MINB>
+template <typename T, int RECON, bool EPI, int MINB, int L3>
 int launch_tile2(nd_ctx* ctx, void* out, const void* in, double m, double s0, double s1, const void* v1, double s2, const void* v2,
                  double s3, const void* v3) {
     using Vec = typename Prec<T>::Vec;
@@ -788,10 +792,10 @@ int launch_tile2(nd_ctx* ctx, void* out, const void* in, double m, double s0, do
     G.V = ctx->V;
     G.S0 = (long long)ctx->dims[1] * ctx->dims[2] * ctx->dims[3];
     G.bc = ctx->bc;
-    G.nt2 = G.L2 / 2;
+    G.nt2 = G.L2 / (2 * (32 / L3));
     G.ntile = (G.L1 / 2) * G.nt2;
-    auto kern = wilson_Q_tile2_kernel<T, RECON, EPI, MINB>;
-    int& per_sm = ctx->tile_ctas_per_sm[EPI ? 1 : 0];
+    auto kern = wilson_Q_tile2_kernel<T, RECON, EPI, MINB, L3>;
+    int& per_sm = ctx->tile_ctas_per_sm[4 + (EPI ? 1 : 0)];
     if (per_sm == 0) {
         ND_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int n = 0;
@@ -845,8 +849,9 @@ int launch_tile(nd_ctx* ctx, void* out, const void* in, double m, double s0, dou
     return ND_OK;
 }
 
-// fp32 only (see ndi_tile_supported).  Registers per thread: the plain kernel fits 3 CTAs of 128 threads per SM (168
-// registers), the fused-epilogue kernel holds the three update vectors of its site as well and runs 2 CTAs per SM.
+// The four-slot kernel, fp32 only (ND_STENCIL_TILE4 / ND_STENCIL_TILE_TMA; the default is the two-slot kernel below, which grew out
+// of it).  Registers per thread: the plain kernel fits 3 CTAs of 128 threads per SM (168 registers), the fused-epilogue kernel
+// holds the three update vectors of its site as well and runs 2 CTAs per SM.
 template <int RECON>
 int launch_tile_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                       const void* v2, double s3, const void* v3) {
@@ -864,29 +869,47 @@ int launch_tile_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi
 }  // namespace
 
 // Lattices the tiled kernels take: x3 extent 32 (tile 2 x 2 x 32: a warp is one x3 row), even x1 / x2 extents, and enough tiles
-// to give every SM work.  fp32: wilson_Q_tile_kernel; fp64: wilson_Q_tile2_kernel (x1, x2 extents >= 4, recon 12 / 8).
+// to give every SM work; x1, x2 extents >= 4 for the two-slot kernel (every site of a tile has exactly one outside neighbour
+// per direction); fp64: recon 12 / 8 only (with 9 link words per slot two CTAs no longer fit an SM).
+// (at least ND_TILE_MIN_CTA_SLICES_PER_SM slices of 128 sites per SM: below that the segments along x0 get so short that their
+// prologue - one extra spinor and link per column - eats the gain; 16^3x32 has 6.9 and runs 12.3 us site vs 14.4 us tiled in fp32)
+constexpr long long ND_TILE_MIN_CTA_SLICES_PER_SM = 8;
 bool ndi_tile_supported(const nd_ctx* ctx) {
     const int L1 = ctx->dims[1], L2 = ctx->dims[2], L3 = ctx->dims[3];
-    if (L3 != 32) return false;
-    if (L1 % 2 != 0 || L2 % 2 != 0) return false;
-    if (ctx->prec == 64 && (L1 < 4 || L2 < 4 || ctx->recon == 18)) return false;
-    return (long long)(L1 / 2) * (L2 / 2) * ctx->dims[0] >= 8LL * ctx->num_sms;
+    if (L3 != 32 && L3 != 16) return false;
+    if (L1 % 2 != 0 || L2 % (64 / L3) != 0) return false;      // x3 extent 16: a CTA takes two tiles side by side in x2
+    if (L1 < 4 || L2 < 4) return false;
+    if (ctx->prec == 64 && ctx->recon == 18) return false;
+    return ctx->V / 128 >= ND_TILE_MIN_CTA_SLICES_PER_SM * ctx->num_sms;
 }
 
-template <int RECON>
+// fp32: 3 CTAs of 128 threads per SM for the plain stencil (145 registers), 2 for the fused epilogue (the three update vectors of
+// the site are loaded before the last barrier); fp64: 2 CTAs per SM (255 registers, 105 KB shared memory)
+template <typename T, int RECON, int MINB, int MINB_EPI>
 static int launch_tile2_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
-                       const void* v2, double s3, const void* v3) {
-    if (epi) return launch_tile2<double, RECON, true, 2>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
-    return launch_tile2<double, RECON, false, 2>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+                              const void* v2, double s3, const void* v3) {
+    if (ctx->dims[3] == 16) {
+        if (epi) return launch_tile2<T, RECON, true, MINB_EPI, 16>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile2<T, RECON, false, MINB, 16>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+    }
+    if (epi) return launch_tile2<T, RECON, true, MINB_EPI, 32>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile2<T, RECON, false, MINB, 32>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
 }
 
+// ND_STENCIL_TILE (and auto): the two-slot kernel wilson_Q_tile2_kernel; ND_STENCIL_TILE4 / ND_STENCIL_TILE_TMA (fp32 only): the
+// four-slot kernel wilson_Q_tile_kernel with cp.async / TMA bulk copies
 int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                      const void* v2, double s3, const void* v3) {
     if (ctx->prec == 64) {
-        if (ctx->recon == 12) return launch_tile2_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
-        return launch_tile2_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        if (ctx->recon == 12) return launch_tile2_shape<double, 12, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile2_shape<double, 8, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
     }
-    if (ctx->recon == 18) return launch_tile_shape<18>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);   // (fused epilogue only)
-    if (ctx->recon == 12) return launch_tile_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
-    return launch_tile_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    if (ctx->stencil_variant == ND_STENCIL_TILE4 || ctx->stencil_variant == ND_STENCIL_TILE_TMA) {
+        if (ctx->recon == 18) return launch_tile_shape<18>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        if (ctx->recon == 12) return launch_tile_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    }
+    if (ctx->recon == 18) return launch_tile2_shape<float, 18, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    if (ctx->recon == 12) return launch_tile2_shape<float, 12, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile2_shape<float, 8, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
 }

@@ -1,7 +1,7 @@
-"""The tiled marching stencil (csrc/wilson_tile.cu: neighbour exchange through shared memory, cp.async / TMA-bulk prefetch)
+"""The tiled marching stencils (csrc/wilson_tile.cu: neighbour exchange through shared memory, cp.async / TMA-bulk prefetch)
 against the CPU oracle of eq. 2.1 and against the site-per-thread kernel, on lattices that exercise its index logic: several
 time segments per tile, the antiperiodic seam inside a segment, tiles on the lattice boundary in x1 / x2, and an x1 extent
-equal to the tile (both x1 neighbours are the same partner row)."""
+of 4 (both outside x1 neighbours of a pair of rows belong to the same neighbouring tile)."""
 import numpy as np
 import pytest
 
@@ -12,7 +12,7 @@ from tests.gpu_common import TOL, make_context, rel_l2, round_to
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("dims,bc", [((40, 8, 16, 32), -1), ((152, 2, 16, 32), -1), ((38, 16, 8, 32), +1)])
+@pytest.mark.parametrize("dims,bc", [((40, 8, 16, 32), -1), ((152, 4, 16, 32), -1), ((38, 16, 8, 32), +1)])
 @pytest.mark.parametrize("recon", [12, 8, 18])
 def test_every_variant_matches_the_oracle(dims, bc, recon):
     ctx, U = make_context(dims, 32, recon, bc, "smooth", eps=0.3)
@@ -25,7 +25,7 @@ def test_every_variant_matches_the_oracle(dims, bc, recon):
     s0, s1, s2, s3 = 0.37, -1.2, -1.0, 0.81
     ref_epi = s0 * ref + s1 * vecs[0] + s2 * vecs[1] + s3 * vecs[2]
     results = {}
-    for variant in ("site", "tile", "tile_tma", "auto"):
+    for variant in ("site", "tile", "tile4", "tile_tma", "auto"):
         ctx.set_stencil_variant(variant)
         ctx.apply_Q(y, x, -1.6)
         got = ctx.unpack_spinor(y)
@@ -35,10 +35,9 @@ def test_every_variant_matches_the_oracle(dims, bc, recon):
         ctx.copy(out, d[1])
         ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])   # out aliases v2, as in the Clenshaw step
         assert rel_l2(ctx.unpack_spinor(out), ref_epi) <= TOL[32], variant
-    # cp.async and TMA prefetch feed the same arithmetic: bit-identical results
-    assert np.array_equal(results["tile"], results["tile_tma"])
-    # auto = the tiled kernel, except for the plain stencil with uncompressed links (the site-per-thread kernel is faster there)
-    assert np.array_equal(results["site" if recon == 18 else "tile"], results["auto"])
+    # cp.async and TMA prefetch feed the same arithmetic, and so do the two- and the four-slot kernel: bit-identical results
+    assert np.array_equal(results["tile4"], results["tile_tma"]) and np.array_equal(results["tile"], results["tile4"])
+    assert np.array_equal(results["tile"], results["auto"])       # auto = the tiled kernel
     # worst site against the oracle, not only the norm
     scale = np.abs(ref).max()
     assert np.abs(results["tile"] - ref).max() <= (2e-5 if recon != 8 else 2e-4) * scale
@@ -74,6 +73,34 @@ def test_fp64_tiled_kernel_matches_the_oracle(dims, bc, recon):
     assert np.array_equal(results["auto"], results["tile"]) and np.array_equal(fused["auto"], fused["site"])
     scale = np.abs(ref).max()
     assert np.abs(results["tile"] - ref).max() <= (1e-13 if recon != 8 else 1e-10) * scale
+
+
+@pytest.mark.parametrize("dims,bc", [((48, 16, 16, 16), -1), ((64, 8, 20, 16), +1)])
+@pytest.mark.parametrize("prec,recon", [(32, 12), (32, 8), (32, 18), (64, 12), (64, 8)])
+def test_x3_extent_16(dims, bc, prec, recon):
+    """x3 extent 16 (BASELINE configs 1 and 4 are 16^3x32): a CTA takes two 2 x 2 x 16 tiles side by side in x2, a warp holds both
+    rows of an x2 pair (the x2 exchange is synchronised within the warp), x3 shuffles stay inside half-warps."""
+    ctx, U = make_context(dims, prec, recon, bc, "smooth", eps=0.3)
+    psi = round_to(gaussian_spinor(dims), prec)
+    vecs = [round_to(gaussian_spinor(dims, seed=20 + i), prec) for i in range(3)]
+    x, y = ctx.pack_spinor(psi), ctx.new_spinor()
+    d = [ctx.pack_spinor(v) for v in vecs]
+    ref = wilson_c.apply_Q(psi, U, -1.6, bc)
+    s0, s1, s2, s3 = 0.37, -1.2, -1.0, 0.81
+    ref_epi = s0 * ref + s1 * vecs[0] + s2 * vecs[1] + s3 * vecs[2]
+    assert ctx.get_stencil_variant() == "tile"
+    for variant in ("site", "tile", "auto"):
+        ctx.set_stencil_variant(variant)
+        ctx.apply_Q(y, x, -1.6)
+        assert rel_l2(ctx.unpack_spinor(y), ref) <= TOL[prec], (variant, rel_l2(ctx.unpack_spinor(y), ref))
+        out = ctx.new_spinor()
+        ctx.copy(out, d[1])
+        ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])
+        assert rel_l2(ctx.unpack_spinor(out), ref_epi) <= TOL[prec], variant
+    import paper_1010_5636_b200 as nd
+    for variant in ("tile4", "tile_tma"):                            # the four-slot kernel exists for x3 extent 32 only
+        with pytest.raises(nd.NDError):
+            ctx.set_stencil_variant(variant)
 
 
 def test_variant_selection_rules():
