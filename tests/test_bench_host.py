@@ -69,10 +69,13 @@ def test_spawn_command_and_traffic_table():
     assert cmd[-4:] == ["--gpus", "4", "--steps", "2"] and cmd[-5].endswith("bench.py")
     assert bench.load_traffic("wilson_Q_kernel", "5^3x7", 32, 12) is None          # no capture of that lattice
     assert bench.load_traffic("no_such_kernel", "32^3x64", 32, 12) is None
-    t = bench.load_traffic("wilson_Q_tile_kernel", "32^3x64", 32, 12)
-    assert t is None or 0.9 * 805306368 < t < 1.3 * 805306368                      # a capture, if present, is near the byte model
+    for kernel, prec in (("wilson_Q_tile2_kernel", 32), ("wilson_Q_tile2_kernel", 64), ("wilson_Q_tile_kernel", 32)):
+        t = bench.load_traffic(kernel, "32^3x64", prec, 12)
+        model = bench.q_bytes_per_site(prec, 12) * 2097152
+        assert t is None or 0.9 * model < t < 1.3 * model                          # a capture, if present, is near the byte model
     assert bench.stencil_kernel_name("site", 8192) == "wilson_Q_hop_kernel" and bench.stencil_kernel_name("site", 1 << 20) == "wilson_Q_kernel"
-    assert bench.stencil_kernel_name("tile", 1 << 21) == "wilson_Q_tile_kernel"
+    assert bench.stencil_kernel_name("tile", 1 << 21) == "wilson_Q_tile2_kernel" and bench.stencil_kernel_name("tile", 1 << 21, 64) == "wilson_Q_tile2_kernel"
+    assert bench.stencil_kernel_name("tile4", 1 << 21) == "wilson_Q_tile_kernel" and bench.stencil_kernel_name("tile_tma", 1 << 21) == "wilson_Q_tile_kernel"
 
 
 def test_reference_arm_other_ranks_exit_without_work():
