@@ -86,7 +86,9 @@ def load_traffic(kernel, lattice, prec, recon):
 def stencil_kernel_name(variant, sites, prec=32):
     if variant == "tile":
         return "wilson_Q_tile2_kernel"
-    if variant in ("tile4", "tile_tma"):
+    if variant == "tile_tma":
+        return "wilson_Q_tile3_kernel"
+    if variant == "tile4":
         return "wilson_Q_tile_kernel"
     return "wilson_Q_hop_kernel" if sites < 16384 else "wilson_Q_kernel"
 
@@ -594,7 +596,7 @@ def run_b200(args):
     for p, r in ((32, 12), (64, 12), (32, 8), (64, 8), (32, 18), (64, 18)):
         if args.quick and (p, r) != (prec, recon):
             continue
-        variants = (None, "site", "tile4", "tile_tma") if p == 32 else (None, "site")
+        variants = (None, "site", "tile_tma", "tile4") if p == 32 else (None, "site", "tile_tma")
         qk[f"f{p}_recon{r}"] = measure_q_kernel(torch, nd, gdims, args.lattice, U64, p, r, peak, variants)
     q_clocks = q_sampler.stop()
     main = qk[f"f{prec}_recon{recon}"]
@@ -696,7 +698,7 @@ def main():
     ap.add_argument("--quick", action="store_true", help="headline + its own Q-kernel variant only (no layout / configs legs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--q-only", action="store_true", help="time only the Q stencil of --prec / --recon on --lattice (plain and fused epilogue)")
-    ap.add_argument("--variant", default=None, choices=["site", "tile", "tile4", "tile_tma"], help="with --q-only: force a stencil variant")
+    ap.add_argument("--variant", default=None, choices=["site", "tile", "tile_tma", "tile4"], help="with --q-only: force a stencil variant")
     ap.add_argument("--replicas", action="store_true", help="--gpus N as N independent lattices (weak scaling) instead of the domain decomposition")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup

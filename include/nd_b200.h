@@ -74,9 +74,10 @@ ND_API size_t nd_gauge_bytes(const nd_ctx* ctx);        /* bytes of the compress
  * picks the fastest one measured for the context and call: the tiled marching kernel (neighbour exchange through shared memory,
  * cp.async prefetch of links, halos and the next spinor) on lattices it supports - x3 extent 32 or 16, even x1 / x2 extents >= 4
  * (x3 extent 16: x2 extent divisible by 4), at least 8 slices of 128 sites per SM, in fp64 recon 12 / 8 and the plain stencil
- * only - and the site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The other values force one kernel for every call, for parity tests and for timing the variants against
- * each other: ND_STENCIL_SITE, ND_STENCIL_TILE (the tiled kernel above), and in fp32 its predecessor with four link slots and
- * the next spinor in registers (x3 extent 32), prefetching by cp.async (ND_STENCIL_TILE4) or by TMA bulk copies (ND_STENCIL_TILE_TMA);
+ * only - and the site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The other values force one kernel for every
+ * call, for parity tests and for timing the variants against each other: ND_STENCIL_SITE; ND_STENCIL_TILE (the tiled kernel
+ * above); ND_STENCIL_TILE_TMA (the same kernel with every prefetch issued as a TMA tensor-map box load instead of cp.async; x3
+ * extent 32); ND_STENCIL_TILE4 (fp32, x3 extent 32: its predecessor with four link slots and the next spinor in registers).
  * ND_ERR_BAD_ARG if the context cannot run it.  Cached CUDA graphs are dropped.  nd_get_stencil_variant returns the variant in
  * effect for the plain stencil (never ND_STENCIL_AUTO). */
 enum { ND_STENCIL_AUTO = 0, ND_STENCIL_SITE = 1, ND_STENCIL_TILE = 2, ND_STENCIL_TILE_TMA = 3, ND_STENCIL_TILE4 = 4 };

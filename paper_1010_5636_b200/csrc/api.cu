@@ -75,7 +75,7 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->num_sms = 148;
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     ctx->err[0] = 0;
-    for (int i = 0; i < 6; i++) ctx->tile_ctas_per_sm[i] = 0;
+    for (int i = 0; i < 8; i++) ctx->tile_ctas_per_sm[i] = 0;
     ctx->tile_ok = ndi_tile_supported(ctx);
     ctx->stencil_variant = ND_STENCIL_AUTO;
     ctx->dot_configured = false;
@@ -142,12 +142,15 @@ extern "C" int nd_set_stencil_variant(nd_ctx* ctx, int variant) {
         return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: unknown variant %d", variant);
     if ((variant == ND_STENCIL_TILE || variant == ND_STENCIL_TILE_TMA || variant == ND_STENCIL_TILE4) && !ctx->tile_ok)
         return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: the tiled kernel needs x3 extent 32 or 16, even x1 / x2 extents >= 4 (x3 extent 16: x2 extent divisible by 4; fp64: recon 12 / 8) and >= 8 slices of 128 sites per SM");
-    if ((variant == ND_STENCIL_TILE_TMA || variant == ND_STENCIL_TILE4) && (ctx->prec != 32 || ctx->dims[3] != 32))
-        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: the four-slot tiled kernel (cp.async / TMA bulk copies) exists in fp32 for x3 extent 32 only");
+    if (variant == ND_STENCIL_TILE4 && (ctx->prec != 32 || ctx->dims[3] != 32))
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: the four-slot tiled kernel exists in fp32 for x3 extent 32 only");
+    if (variant == ND_STENCIL_TILE_TMA && ctx->dims[3] != 32)
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_stencil_variant: the tensor-map tiled kernel exists for x3 extent 32 only");
     ctx->stencil_variant = variant;
     ndi_drop_graphs(ctx);
     return ND_OK;
 }
+
 extern "C" int nd_get_stencil_variant(const nd_ctx* ctx) {
     if (!ctx) return ND_ERR_BAD_ARG;
     if (ctx->stencil_variant != ND_STENCIL_AUTO) return ctx->stencil_variant;

@@ -63,7 +63,7 @@ struct nd_ctx {
     bool dot_configured;        // block_dot_cols_kernel shared-memory attributes set
     bool tile_ok;               // the tiled marching stencil (wilson_tile.cu) takes this lattice
     int stencil_variant;        // ND_STENCIL_* (nd_set_stencil_variant)
-    int tile_ctas_per_sm[6];    // resident CTAs per SM of the tiled kernels ({cp.async, TMA, two-slot} x {plain, fused}), 0 = not queried yet
+    int tile_ctas_per_sm[8];    // resident CTAs per SM of the tiled kernels ({four-slot, -, two-slot, tensor map} x {plain, fused}), 0 = not queried yet
     // domain decomposition along x0 (shard.cu): this context is the local lattice of rank shard_rank of shard_n
     int shard_rank, shard_n;
     bool in_shard_call;         // the local stencil of a sharded application is being enqueued

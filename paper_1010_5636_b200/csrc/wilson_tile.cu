@@ -20,6 +20,8 @@
 //   * x1 and x2 use separate exchange buffers in turn (send x1, barrier, receive x1, send x2, barrier, receive x2): two
 //     __syncthreads per time-slice and no buffer is ever written while it may still be read.
 // L2 -> SM traffic per site (fp32, recon 12, tile 2 x 4 x 32): 288 own + 96 store + 180 halo = 564 B; tile 4 x 4 x 32: 504 B.
+#include <cuda.h>   // CUtensorMap (the tensor-map variant at the end of this file)
+
 #include "nd_dirac.cuh"
 
 namespace {
@@ -115,20 +117,13 @@ template <int BYTES> __device__ __forceinline__ void cp_async(void* smem_dst, co
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// TMA bulk copies (cp.async.bulk, SASS UBLKCP): a warp owns one x3 row of 32 sites, and every plane of that row is 32
-// consecutive 128-bit words both in global memory and in the row's shared-memory slot, so one lane moves a whole row-plane
-// (512 bytes) with one instruction; completion is counted in bytes on an mbarrier of the warp.
+// mbarrier helpers of the tensor-map variant (wilson_Q_tile3_kernel): completion of TMA loads is counted in bytes
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
 }
 __device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
-                 "r"(bytes), "r"(smem_u32(b))
-                 : "memory");
 }
 __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
     asm volatile(
@@ -164,33 +159,6 @@ __device__ __forceinline__ void issue_halo(unsigned char* hal, const typename Pr
 #pragma unroll
         for (int p = 0; p < LL::NL; p++) cp_async<sizeof(typename LL::LVec)>(&hl[p * HLN + hidx], gauge + ((long long)MU * LL::NL + p) * V + s_bwd);
     }
-}
-
-// the same with bulk copies: lanes 0..NV-1 move one spinor plane of the neighbour row each, lanes NV..NV+NL-1 one link word
-// (rows are warp-uniform: L3 = 32).  Returns the bytes issued (for the mbarrier's expect_tx, armed by the caller).
-template <typename T, int RECON, int MU, int NT>
-__device__ __forceinline__ void issue_halo_bulk(unsigned char* hal, const typename Prec<T>::Vec* __restrict__ in,
-                                                const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, long long V, int row0,
-                                                int lane, bool face_bwd, bool face_fwd, long long row_bwd, long long row_fwd,
-                                                unsigned long long* bar) {
-    using Vec = typename Prec<T>::Vec;
-    using LL = LinkLayout<T, RECON>;
-    Vec* hs = reinterpret_cast<Vec*>(hal);
-    typename LL::LVec* hl = reinterpret_cast<typename LL::LVec*>(hal + (size_t)Prec<T>::NV * NT * sizeof(Vec));
-    if (face_fwd || face_bwd) {
-        const long long sn = face_fwd ? row_fwd : row_bwd;
-        if (lane < Prec<T>::NV) bulk_g2s(&hs[lane * NT + row0], in + lane * V + sn, 32 * sizeof(Vec), bar);
-        else if (face_bwd && lane < Prec<T>::NV + LL::NL)
-            bulk_g2s(&hl[(lane - Prec<T>::NV) * NT + row0], gauge + ((long long)MU * LL::NL + (lane - Prec<T>::NV)) * V + row_bwd,
-                     32 * sizeof(typename LL::LVec), bar);
-    }
-}
-template <typename T, int RECON> __device__ __forceinline__ unsigned halo_bytes(bool face_bwd, bool face_fwd) {
-    using LL = LinkLayout<T, RECON>;
-    unsigned b = 0;
-    if (face_fwd || face_bwd) b += Prec<T>::NV * 32 * sizeof(typename Prec<T>::Vec);
-    if (face_bwd && !face_fwd) b += LL::NL * 32 * sizeof(typename LL::LVec);
-    return b;
 }
 
 // One direction mu in {1, 2} of the send phase of a site: the two half-spinors its in-tile neighbours need, and, on a tile
@@ -264,22 +232,6 @@ __device__ __forceinline__ void take_link(typename LinkLayout<T, RECON>::LVec* l
     }
 }
 
-// bulk variant: lanes 0..NL-1 refill one row-plane of the slot each (the whole warp has read its words before: __syncwarp)
-template <typename T, int RECON, int NT>
-__device__ __forceinline__ void take_link_bulk(typename LinkLayout<T, RECON>::LVec* lnk, const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge,
-                                               long long V, int mu, int site, int lane, bool refill, long long row_next,
-                                               unsigned long long* bar, cx<T> (&U)[3][3]) {
-    using LL = LinkLayout<T, RECON>;
-    typename LL::LVec w[LL::NL];
-#pragma unroll
-    for (int p = 0; p < LL::NL; p++) w[p] = lnk[(mu * LL::NL + p) * NT + site];
-    reconstruct_link<T, RECON>(w, U);
-    __syncwarp();
-    if (refill && lane < LL::NL)
-        bulk_g2s(&lnk[(mu * LL::NL + lane) * NT + (site - lane)], gauge + ((long long)mu * LL::NL + lane) * V + row_next,
-                 32 * sizeof(typename LL::LVec), bar);
-}
-
 // The vectors of the fused update out = s0*Q(in) + s1*v1 + s2*v2 + s3*v3 at this thread's site, loaded BEFORE the last barrier
 // of the slice and combined after it (out may alias any v_i: every v_i(x) is read before out(x) is written, by the same thread).
 // (fp64 has no registers to spare for this: there the vectors are loaded at use, after the barrier.)
@@ -349,7 +301,7 @@ template <typename T, bool EPI> struct EpiVectors {
 template <int B1, int B2, int L3> struct PairSync { static constexpr bool value = (B1 == 2 && B2 == 2 && L3 == 32); };
 __device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 
-template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB, bool BULK>
+template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB>
 __global__ void __launch_bounds__(B1* B2* L3, MINB)
     wilson_Q_tile_kernel(typename Prec<T>::Vec* out, const typename Prec<T>::Vec* __restrict__ in,
                          const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, TileGeom G, T mass_term, T s0, T s1,
@@ -379,29 +331,13 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
     const int ts = seg * G.seg_base + (seg < G.seg_rem ? seg : G.seg_rem);
     const int len = G.seg_base + (seg < G.seg_rem ? 1 : 0);
 
-    // bulk mode: two mbarriers per warp - TOP: the next slice's four links and x1 halo; MID: this slice's x2 halo
-    __shared__ unsigned long long mbar[2][NT / 32];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    unsigned long long* bar_top = &mbar[0][warp];
-    unsigned long long* bar_mid = &mbar[1][warp];
-    const int row0 = site - lane;                  // the row's first slot (BULK: L3 == 32, lane == x3)
-    const long long rr = ss - lane;                // ... and first site within a slice
-    if (BULK) {
-        if (lane == 0) { mbar_init(bar_top, 1); mbar_init(bar_mid, 1); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        __syncthreads();
-    }
+    const int lane = threadIdx.x & 31;
     // the links of the segment's first slice start their way into the thread's slot
-    if (BULK) {
-        for (int j = lane; j < 4 * LL::NL; j += 32)   // (recon 18 has 36 row-planes)
-            bulk_g2s(&lnk[j * NT + row0], gauge + (long long)j * G.V + ts * G.S0 + rr, 32 * sizeof(LVec), bar_top);
-    } else {
 #pragma unroll
-        for (int mu = 0; mu < 4; mu++)
+    for (int mu = 0; mu < 4; mu++)
 #pragma unroll
-            for (int p = 0; p < LL::NL; p++)
-                cp_async<sizeof(LVec)>(&lnk[(mu * LL::NL + p) * NT + site], gauge + ((long long)mu * LL::NL + p) * G.V + ts * G.S0 + ss);
-    }
+        for (int p = 0; p < LL::NL; p++)
+            cp_async<sizeof(LVec)>(&lnk[(mu * LL::NL + p) * NT + site], gauge + ((long long)mu * LL::NL + p) * G.V + ts * G.S0 + ss);
 
     // neighbours in x1 / x2: inside the tile (slot index), or outside (global site offset within the slice)
     const bool wrap1 = (G.L1 == B1), wrap2 = (G.L2 == B2);
@@ -418,14 +354,8 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
     const int lane_f3 = (lane & ~(L3 - 1)) | ((lane + 1) & (L3 - 1));
     const int lane_b3 = (lane & ~(L3 - 1)) | ((lane + L3 - 1) & (L3 - 1));
 
-    const unsigned top_bytes = 4 * LL::NL * 32 * sizeof(LVec) + halo_bytes<T, RECON>(face_b1, face_f1);
-    if (BULK) {
-        issue_halo_bulk<T, RECON, 1, NT>(hal, in, gauge, G.V, row0, lane, face_b1, face_f1, ts * G.S0 + ss_b1 - lane, ts * G.S0 + ss_f1 - lane, bar_top);
-        if (lane == 0) mbar_expect_tx(bar_top, top_bytes);
-    } else {
-        issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, ts * G.S0 + ss_b1, ts * G.S0 + ss_f1, site);
-        cp_async_commit();
-    }
+    issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, ts * G.S0 + ss_b1, ts * G.S0 + ss_f1, site);
+    cp_async_commit();
 
     cx<T> phi_c[12], w0[2][3];
     {
@@ -448,12 +378,7 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
         cx<T> phi_n[12];
         load_spinor<T>(in, G.V, ((t == G.L0 - 1) ? 0 : st + G.S0) + ss, phi_n);   // next slice of this column
         // this slice's link words and x1 halo (issued one slice ago) have landed
-        if (BULK) {
-            mbar_wait(bar_top, i & 1);
-            if (more && lane == 0) mbar_expect_tx(bar_top, top_bytes);   // armed for the refills issued during this slice
-        } else {
-            cp_async_wait_all();
-        }
+        cp_async_wait_all();
 
         cx<T> acc[12];
         {
@@ -466,25 +391,17 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
         if (PairSync<B1, B2, L3>::value) pair_barrier(1 + r2);   // the partner row has finished last slice's x1 receive
         {
             cx<T> U[3][3];
-            if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 1, site, lane, more, s_next - lane, bar_top, U);
-            else take_link<T, RECON, NT>(lnk, gauge, G.V, 1, site, more, s_next, U);
+            take_link<T, RECON, NT>(lnk, gauge, G.V, 1, site, more, s_next, U);
             kept.keep(U);
             send_dir<T, RECON, 1, NT, 0>(xbuf, hal, phi_c, U, site, slot_b1, slot_f1, face_b1, face_f1, site);
             // the halo slot is free again: this slice's x2 halo
-            if (BULK) {
-                __syncwarp();
-                issue_halo_bulk<T, RECON, 2, NT>(hal, in, gauge, G.V, row0, lane, face_b2, face_f2, st + ss_b2 - lane, st + ss_f2 - lane, bar_mid);
-                if (lane == 0) mbar_expect_tx(bar_mid, halo_bytes<T, RECON>(face_b2, face_f2));
-            } else {
-                issue_halo<T, RECON, 2, NT>(hal, in, gauge, G.V, site, face_b2, face_f2, st + ss_b2, st + ss_f2, site);
-                cp_async_commit();
-            }
+            issue_halo<T, RECON, 2, NT>(hal, in, gauge, G.V, site, face_b2, face_f2, st + ss_b2, st + ss_f2, site);
+            cp_async_commit();
         }
         // ---- x3: the neighbours are lanes of this warp
         {
             cx<T> U[3][3], h[2][3], g[2][3];
-            if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 3, site, lane, more, s_next - lane, bar_top, U);
-            else take_link<T, RECON, NT>(lnk, gauge, G.V, 3, site, more, s_next, U);
+            take_link<T, RECON, NT>(lnk, gauge, G.V, 3, site, more, s_next, U);
             project<T, 3, -1>(phi_c, T(1), h);
             shfl_half(h, lane_f3);             // (1 - gamma_3) phi(x + 3^)
             mul_U(U, h, g);
@@ -505,36 +422,25 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
         if (PairSync<B1, B2, L3>::value) pair_barrier(3 + r1);   // the partner row has finished last slice's x2 receive
         {
             cx<T> U[3][3];
-            if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 2, site, lane, more, s_next - lane, bar_top, U);
-            else take_link<T, RECON, NT>(lnk, gauge, G.V, 2, site, more, s_next, U);
+            take_link<T, RECON, NT>(lnk, gauge, G.V, 2, site, more, s_next, U);
             kept.keep(U);
             // the x2 halo
-            if (BULK) mbar_wait(bar_mid, i & 1);
-            else cp_async_wait_all();
+            cp_async_wait_all();
             send_dir<T, RECON, 2, NT, K2>(xbuf, hal, phi_c, U, site, slot_b2, slot_f2, face_b2, face_f2, site);
-            if (more) {
-                if (BULK) {
-                    __syncwarp();
-                    issue_halo_bulk<T, RECON, 1, NT>(hal, in, gauge, G.V, row0, lane, face_b1, face_f1, st + G.S0 + ss_b1 - lane,
-                                                     st + G.S0 + ss_f1 - lane, bar_top);
-                } else {
-                    issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, st + G.S0 + ss_b1, st + G.S0 + ss_f1, site);
-                }
-            }
+            if (more) issue_halo<T, RECON, 1, NT>(hal, in, gauge, G.V, site, face_b1, face_f1, st + G.S0 + ss_b1, st + G.S0 + ss_f1, site);
         }
         // ---- x0: this thread's own column
         {
             cx<T> U[3][3], h[2][3], g[2][3];
             accumulate<T, 0, +1>(w0, acc);     // carried from the previous slice
-            if (BULK) take_link_bulk<T, RECON, NT>(lnk, gauge, G.V, 0, site, lane, more, s_next - lane, bar_top, U);
-            else take_link<T, RECON, NT>(lnk, gauge, G.V, 0, site, more, s_next, U);
+            take_link<T, RECON, NT>(lnk, gauge, G.V, 0, site, more, s_next, U);
             project<T, 0, -1>(phi_n, (t == G.L0 - 1) ? T(G.bc) : T(1), h);
             mul_U(U, h, g);
             accumulate<T, 0, -1>(g, acc);
             project<T, 0, +1>(phi_c, (t == G.L0 - 1) ? T(G.bc) : T(1), h);
             mul_Udag(U, h, w0);                // the next slice's backward time hop
         }
-        if (!BULK) cp_async_commit();
+        cp_async_commit();
         EpiVectors<T, EPI> ev;
         ev.load(G.V, s, s1, v1, s2, v2, s3, v3);   // the fused update's vectors are on their way while the barrier is met
         if (PairSync<B1, B2, L3>::value) pair_barrier(3 + r1);   // x2 half-spinors are in place
@@ -813,7 +719,331 @@ int launch_tile2(nd_ctx* ctx, void* out, const void* in, double m, double s0, do
     return ND_OK;
 }
 
-template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB, bool BULK>
+// ------------------------------------------------------------------------------ the tensor-map (TMA) variant
+// wilson_Q_tile2_kernel with every prefetch issued as a TMA tensor-map box load (cp.async.bulk.tensor.5d, SASS UTMALDG) instead of
+// per-thread cp.async: the spinor and link arrays are described to the TMA unit as 5D tensors
+//     [plane][x0][x1][x2][x3 row of 32 128-bit words]     (plane stride = one lattice volume)
+// and ONE request moves all planes of one x3 row (a box of 1 x 1 x 1 x 1 row x NP planes: 1.5 KB for a link, 3 KB for a spinor in
+// fp32) into the warp's private slot, laid out [plane][lane].  A warp is one row, so lane 0 of every warp issues for its own row
+// after a __syncwarp (all lanes have read the slot) and completion is counted in bytes on four mbarriers per warp, one per group
+// of the two-slot schedule above: at most 9 requests per warp and slice (plain bulk copies, one per row-plane, would be 21 of 512
+// bytes) and no LDGSTS, no per-thread address arithmetic.  Periodic wrap-around is in the box coordinates.  fp32 / fp64, x3
+// extent 32.
+struct TileMaps {
+    CUtensorMap spinor;   // `in`
+    CUtensorMap links;    // the context's gauge field
+};
+__device__ __forceinline__ void tma_row(void* dst, const CUtensorMap* tm, int x2, int x1, int x0, int plane0, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(tm), "r"(0), "r"(x2), "r"(x1), "r"(x0), "r"(plane0), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+template <typename T, int RECON, bool EPI, int MINB>
+__global__ void __launch_bounds__(128, MINB)
+    wilson_Q_tile3_kernel(typename Prec<T>::Vec* out, const typename Prec<T>::Vec* __restrict__ in,
+                          const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, const __grid_constant__ TileMaps maps,
+                          TileGeom G, T mass_term, T s0, T s1, const typename Prec<T>::Vec* v1, T s2, const typename Prec<T>::Vec* v2,
+                          T s3, const typename Prec<T>::Vec* v3) {
+    using Vec = typename Prec<T>::Vec;
+    using LL = LinkLayout<T, RECON>;
+    using LVec = typename LL::LVec;
+    constexpr int L3 = 32, NT = 128, NL = LL::NL;
+    constexpr int NW = HalfWords<T>::NW, NV = Prec<T>::NV;
+    constexpr int ROW1 = 2 * L3, ROW2 = L3;
+    constexpr unsigned LROW = NL * 32 * sizeof(LVec), SROW = NV * 32 * sizeof(Vec);   // bytes of one link / spinor row box
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    unsigned char* sp = smem_raw;
+    Vec* xbuf = reinterpret_cast<Vec*>(sp);   sp += (size_t)2 * NW * NT * sizeof(Vec);   // exchange: [2 kinds][NW][NT]
+    LVec* lnkA = reinterpret_cast<LVec*>(sp); sp += (size_t)NL * NT * sizeof(LVec);      // per warp [NL][32]: x1, then x2
+    LVec* lnkB = reinterpret_cast<LVec*>(sp); sp += (size_t)NL * NT * sizeof(LVec);      // x3, then x0
+    Vec* hals = reinterpret_cast<Vec*>(sp);   sp += (size_t)NV * NT * sizeof(Vec);       // halo spinor, per warp [NV][32]
+    LVec* hall = reinterpret_cast<LVec*>(sp); sp += (size_t)NL * NT * sizeof(LVec);      // halo link (backward faces)
+    Vec* phis = reinterpret_cast<Vec*>(sp);                                               // next spinor of the column
+    __shared__ unsigned long long mbar[4][NT / 32];
+
+    const int site = threadIdx.x, lane = site & 31, warp = site >> 5;
+    const int x3 = lane, r2 = warp & 1, r1 = warp >> 1;
+    const int tile = blockIdx.x % G.ntile, seg = blockIdx.x / G.ntile;
+    const int x1 = (tile / G.nt2) * 2 + r1, x2 = (tile % G.nt2) * 2 + r2;
+    const long long ss = ((long long)x1 * G.L2 + x2) * L3 + x3;
+    const int ts = seg * G.seg_base + (seg < G.seg_rem ? seg : G.seg_rem);
+    const int len = G.seg_base + (seg < G.seg_rem ? 1 : 0);
+    const bool face_b1 = (r1 == 0), face_f1 = !face_b1, face_b2 = (r2 == 0), face_f2 = !face_b2;
+    const int slot_b1 = face_b1 ? -1 : site - ROW1, slot_f1 = face_f1 ? -1 : site + ROW1;
+    const int slot_b2 = face_b2 ? -1 : site - ROW2, slot_f2 = face_f2 ? -1 : site + ROW2;
+    const int x1n = face_b1 ? (x1 == 0 ? G.L1 - 1 : x1 - 1) : (x1 == G.L1 - 1 ? 0 : x1 + 1);   // the row outside the tile in x1
+    const int x2n = face_b2 ? (x2 == 0 ? G.L2 - 1 : x2 - 1) : (x2 == G.L2 - 1 ? 0 : x2 + 1);   // ... and in x2
+    const int lane_f3 = (lane + 1) & 31, lane_b3 = (lane + 31) & 31;
+    // this warp's private rows in the slots
+    LVec* myA = lnkA + warp * NL * 32;
+    LVec* myB = lnkB + warp * NL * 32;
+    Vec* myhs = hals + warp * NV * 32;
+    LVec* myhl = hall + warp * NL * 32;
+    Vec* myphi = phis + warp * NV * 32;
+    unsigned long long* barA = &mbar[0][warp];   // link 1 + x1 halo
+    unsigned long long* barB = &mbar[1][warp];   // link 3 + next spinor
+    unsigned long long* bar1 = &mbar[2][warp];   // link 2 + x2 halo
+    unsigned long long* bar2 = &mbar[3][warp];   // link 0
+    const unsigned bytesA = LROW + SROW + (face_b1 ? LROW : 0u), bytes1 = LROW + SROW + (face_b2 ? LROW : 0u);
+    if (lane == 0) {
+        mbar_init(barA, 1); mbar_init(barB, 1); mbar_init(bar1, 1); mbar_init(bar2, 1);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+    if (lane == 0) {
+        mbar_expect_tx(barA, bytesA);
+        tma_row(myA, &maps.links, x2, x1, ts, 1 * NL, barA);
+        tma_row(myhs, &maps.spinor, x2, x1n, ts, 0, barA);
+        if (face_b1) tma_row(myhl, &maps.links, x2, x1n, ts, 1 * NL, barA);
+        mbar_expect_tx(barB, LROW + SROW);
+        tma_row(myB, &maps.links, x2, x1, ts, 3 * NL, barB);
+        tma_row(myphi, &maps.spinor, x2, x1, (ts == G.L0 - 1) ? 0 : ts + 1, 0, barB);
+    }
+
+    cx<T> phi_c[12], w0[2][3];
+    {
+        const int tp = (ts == 0) ? G.L0 - 1 : ts - 1;
+        cx<T> psi[12], U[3][3], h[2][3];
+        load_spinor<T>(in, G.V, tp * G.S0 + ss, psi);
+        load_link<T, RECON>(gauge, G.V, 0, tp * G.S0 + ss, U);
+        project<T, 0, +1>(psi, (ts == 0) ? T(G.bc) : T(1), h);
+        mul_Udag(U, h, w0);
+        load_spinor<T>(in, G.V, ts * G.S0 + ss, phi_c);
+    }
+
+    for (int i = 0; i < len; i++) {
+        const int t = ts + i;
+        const long long s = t * G.S0 + ss;
+        const bool more = (i + 1 < len);
+        const unsigned par = i & 1;
+        mbar_wait(barA, par);                      // link 1 and the x1 halo of this slice
+        cx<T> acc[12];
+        {
+            const T f = T(-2) * mass_term;
+#pragma unroll
+            for (int k = 0; k < 12; k++) acc[k] = {f * phi_c[k].re, f * phi_c[k].im};
+        }
+        KeptLink<T> kept;
+        // ---- x1: send
+        pair_barrier(1 + r2);
+        {
+            cx<T> U[3][3], h[2][3], g[2][3];
+            {
+                LVec w[NL];
+#pragma unroll
+                for (int p = 0; p < NL; p++) w[p] = myA[p * 32 + lane];
+                reconstruct_link<T, RECON>(w, U);
+            }
+            kept.keep(U);
+            if (!face_b1) { project<T, 1, -1>(phi_c, T(1), h); put_half<T, NT>(xbuf, 0, slot_b1, h); }
+            if (!face_f1) { project<T, 1, +1>(phi_c, T(1), h); mul_Udag(U, h, g); put_half<T, NT>(xbuf, 1, slot_f1, g); }
+            {
+                Vec w[NV];
+#pragma unroll
+                for (int p = 0; p < NV; p++) w[p] = myhs[p * 32 + lane];
+                cx<T> psi[12];
+                words_to_cx(w, psi);
+                if (face_f1) { project<T, 1, -1>(psi, T(1), h); put_half<T, NT>(xbuf, 0, site, h); }
+                else {
+                    LVec lw[NL];
+#pragma unroll
+                    for (int p = 0; p < NL; p++) lw[p] = myhl[p * 32 + lane];
+                    cx<T> Ub[3][3];
+                    reconstruct_link<T, RECON>(lw, Ub);
+                    project<T, 1, +1>(psi, T(1), h);
+                    mul_Udag(Ub, h, g);
+                    put_half<T, NT>(xbuf, 1, site, g);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) {                       // group 1: link 2 and the x2 halo of this slice
+                mbar_expect_tx(bar1, bytes1);
+                tma_row(myA, &maps.links, x2, x1, t, 2 * NL, bar1);
+                tma_row(myhs, &maps.spinor, x2n, x1, t, 0, bar1);
+                if (face_b2) tma_row(myhl, &maps.links, x2n, x1, t, 2 * NL, bar1);
+            }
+        }
+        // ---- x3: lanes of this warp
+        mbar_wait(barB, par);                      // link 3 (and the next spinor of the column)
+        {
+            cx<T> U[3][3], h[2][3], g[2][3];
+            {
+                LVec w[NL];
+#pragma unroll
+                for (int p = 0; p < NL; p++) w[p] = myB[p * 32 + lane];
+                reconstruct_link<T, RECON>(w, U);
+            }
+            __syncwarp();
+            if (lane == 0) {                       // group 2: link 0 of this slice
+                mbar_expect_tx(bar2, LROW);
+                tma_row(myB, &maps.links, x2, x1, t, 0, bar2);
+            }
+            project<T, 3, -1>(phi_c, T(1), h);
+            shfl_half(h, lane_f3);
+            mul_U(U, h, g);
+            accumulate<T, 3, -1>(g, acc);
+            project<T, 3, +1>(phi_c, T(1), h);
+            mul_Udag(U, h, g);
+            shfl_half(g, lane_b3);
+            accumulate<T, 3, +1>(g, acc);
+        }
+        pair_barrier(1 + r2);                      // x1 half-spinors are in place
+        {
+            cx<T> U[3][3];
+            kept.get(U);
+            recv_dir<T, 1, NT, 0>(xbuf, U, site, acc);
+        }
+        // ---- x2: send
+        pair_barrier(3 + r1);
+        mbar_wait(bar1, par);                      // link 2 and the x2 halo
+        {
+            cx<T> U[3][3], h[2][3], g[2][3];
+            {
+                LVec w[NL];
+#pragma unroll
+                for (int p = 0; p < NL; p++) w[p] = myA[p * 32 + lane];
+                reconstruct_link<T, RECON>(w, U);
+            }
+            kept.keep(U);
+            if (!face_b2) { project<T, 2, -1>(phi_c, T(1), h); put_half<T, NT>(xbuf, 0, slot_b2, h); }
+            if (!face_f2) { project<T, 2, +1>(phi_c, T(1), h); mul_Udag(U, h, g); put_half<T, NT>(xbuf, 1, slot_f2, g); }
+            {
+                Vec w[NV];
+#pragma unroll
+                for (int p = 0; p < NV; p++) w[p] = myhs[p * 32 + lane];
+                cx<T> psi[12];
+                words_to_cx(w, psi);
+                if (face_f2) { project<T, 2, -1>(psi, T(1), h); put_half<T, NT>(xbuf, 0, site, h); }
+                else {
+                    LVec lw[NL];
+#pragma unroll
+                    for (int p = 0; p < NL; p++) lw[p] = myhl[p * 32 + lane];
+                    cx<T> Ub[3][3];
+                    reconstruct_link<T, RECON>(lw, Ub);
+                    project<T, 2, +1>(psi, T(1), h);
+                    mul_Udag(Ub, h, g);
+                    put_half<T, NT>(xbuf, 1, site, g);
+                }
+            }
+            __syncwarp();
+            if (more && lane == 0) {               // group 3: link 1 and the x1 halo of the next slice
+                mbar_expect_tx(barA, bytesA);
+                tma_row(myA, &maps.links, x2, x1, t + 1, 1 * NL, barA);
+                tma_row(myhs, &maps.spinor, x2, x1n, t + 1, 0, barA);
+                if (face_b1) tma_row(myhl, &maps.links, x2, x1n, t + 1, 1 * NL, barA);
+            }
+        }
+        // ---- x0: this thread's own column
+        mbar_wait(bar2, par);                      // link 0
+        {
+            cx<T> U[3][3], h[2][3], g[2][3];
+            const T ph = (t == G.L0 - 1) ? T(G.bc) : T(1);
+            accumulate<T, 0, +1>(w0, acc);
+            {
+                LVec w[NL];
+#pragma unroll
+                for (int p = 0; p < NL; p++) w[p] = myB[p * 32 + lane];
+                reconstruct_link<T, RECON>(w, U);
+            }
+            project<T, 0, +1>(phi_c, ph, h);
+            mul_Udag(U, h, w0);
+            {
+                Vec w[NV];
+#pragma unroll
+                for (int p = 0; p < NV; p++) w[p] = myphi[p * 32 + lane];
+                words_to_cx(w, phi_c);             // phi(t + 1)
+            }
+            __syncwarp();
+            if (more && lane == 0) {               // group 4: link 3 of the next slice, phi(t + 2)
+                mbar_expect_tx(barB, LROW + SROW);
+                tma_row(myB, &maps.links, x2, x1, t + 1, 3 * NL, barB);
+                tma_row(myphi, &maps.spinor, x2, x1, (t + 1 == G.L0 - 1) ? 0 : t + 2, 0, barB);
+            }
+            project<T, 0, -1>(phi_c, ph, h);
+            mul_U(U, h, g);
+            accumulate<T, 0, -1>(g, acc);
+        }
+        EpiVectors<T, EPI> ev;
+        ev.load(G.V, s, s1, v1, s2, v2, s3, v3);
+        pair_barrier(3 + r1);                      // x2 half-spinors are in place
+        {
+            cx<T> U[3][3];
+            kept.get(U);
+            recv_dir<T, 2, NT, 0>(xbuf, U, site, acc);
+        }
+        ev.finish(out, G.V, s, acc, s0, s1, s2, s3);
+    }
+}
+
+// tensor map of a plane-SoA array of 128-bit (or 64-bit: fp32 recon 18) words: dims (fastest first) reals of an x3 row, x2, x1, x0,
+// planes; box = one x3 row x `box_planes` planes
+typedef CUresult (*nd_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                       CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+int make_row_map(nd_ctx* ctx, CUtensorMap* tm, const void* base, int word_bytes, int planes, int box_planes) {
+    static nd_encode_tiled_fn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        ND_CUDA(ctx, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+        if (!fn || q != cudaDriverEntryPointSuccess) return nd_fail(ctx, ND_ERR_CUDA, "cuTensorMapEncodeTiled is not available in this driver");
+        encode = (nd_encode_tiled_fn)fn;
+    }
+    const int rb = ctx->prec / 8;                                   // bytes of a real
+    const cuuint64_t row = (cuuint64_t)ctx->dims[3] * word_bytes;   // bytes of an x3 row of one plane
+    const cuuint64_t dims[5] = {row / rb, (cuuint64_t)ctx->dims[2], (cuuint64_t)ctx->dims[1], (cuuint64_t)ctx->dims[0], (cuuint64_t)planes};
+    const cuuint64_t strides[4] = {row, row * ctx->dims[2], row * ctx->dims[2] * ctx->dims[1], (cuuint64_t)ctx->V * word_bytes};
+    const cuuint32_t box[5] = {(cuuint32_t)(row / rb), 1, 1, 1, (cuuint32_t)box_planes};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = encode(tm, ctx->prec == 32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<void*>(base),
+                              dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return nd_fail(ctx, ND_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return ND_OK;
+}
+
+template <typename T, int RECON, bool EPI, int MINB>
+int launch_tile3(nd_ctx* ctx, void* out, const void* in, double m, double s0, double s1, const void* v1, double s2, const void* v2,
+                 double s3, const void* v3) {
+    using Vec = typename Prec<T>::Vec;
+    using LL = LinkLayout<T, RECON>;
+    using LVec = typename LL::LVec;
+    constexpr int NT = 128;
+    constexpr size_t smem = (size_t)2 * HalfWords<T>::NW * NT * sizeof(Vec) + (size_t)3 * LL::NL * NT * sizeof(LVec) +
+                            (size_t)2 * Prec<T>::NV * NT * sizeof(Vec);
+    TileGeom G;
+    G.L0 = ctx->dims[0]; G.L1 = ctx->dims[1]; G.L2 = ctx->dims[2];
+    G.V = ctx->V;
+    G.S0 = (long long)ctx->dims[1] * ctx->dims[2] * ctx->dims[3];
+    G.bc = ctx->bc;
+    G.nt2 = G.L2 / 2;
+    G.ntile = (G.L1 / 2) * G.nt2;
+    TileMaps maps;
+    int rc = make_row_map(ctx, &maps.spinor, in, (int)sizeof(Vec), Prec<T>::NV, Prec<T>::NV);
+    if (rc == ND_OK) rc = make_row_map(ctx, &maps.links, ctx->gauge, (int)sizeof(LVec), 4 * LL::NL, LL::NL);
+    if (rc != ND_OK) return rc;
+    auto kern = wilson_Q_tile3_kernel<T, RECON, EPI, MINB>;
+    int& per_sm = ctx->tile_ctas_per_sm[6 + (EPI ? 1 : 0)];
+    if (per_sm == 0) {
+        ND_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int n = 0;
+        ND_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, NT, smem));
+        if (n < 1) return nd_fail(ctx, ND_ERR_CUDA, "tensor-map stencil does not fit on an SM");
+        per_sm = n;
+    }
+    const int nseg = choose_segments(G.L0, G.ntile, per_sm * ctx->num_sms);
+    G.seg_base = G.L0 / nseg;
+    G.seg_rem = G.L0 % nseg;
+    const unsigned blocks = (unsigned)(G.ntile * nseg);
+    kern<<<blocks, NT, smem, ctx->stream>>>((Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, maps, G, T(4.0 + m), T(s0), T(s1),
+                                            (const Vec*)v1, T(s2), (const Vec*)v2, T(s3), (const Vec*)v3);
+    ND_LAUNCHED(ctx);
+    return ND_OK;
+}
+
+template <typename T, int RECON, bool EPI, int B1, int B2, int L3, int MINB>
 int launch_tile(nd_ctx* ctx, void* out, const void* in, double m, double s0, double s1, const void* v1, double s2, const void* v2,
                 double s3, const void* v3) {
     using Vec = typename Prec<T>::Vec;
@@ -830,8 +1060,8 @@ int launch_tile(nd_ctx* ctx, void* out, const void* in, double m, double s0, dou
     G.bc = ctx->bc;
     G.nt2 = G.L2 / B2;
     G.ntile = (G.L1 / B1) * G.nt2;
-    auto kern = wilson_Q_tile_kernel<T, RECON, EPI, B1, B2, L3, MINB, BULK>;
-    int& per_sm = ctx->tile_ctas_per_sm[(BULK ? 2 : 0) + (EPI ? 1 : 0)];
+    auto kern = wilson_Q_tile_kernel<T, RECON, EPI, B1, B2, L3, MINB>;
+    int& per_sm = ctx->tile_ctas_per_sm[EPI ? 1 : 0];
     if (per_sm == 0) {
         ND_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int n = 0;
@@ -849,21 +1079,16 @@ int launch_tile(nd_ctx* ctx, void* out, const void* in, double m, double s0, dou
     return ND_OK;
 }
 
-// The four-slot kernel, fp32 only (ND_STENCIL_TILE4 / ND_STENCIL_TILE_TMA; the default is the two-slot kernel below, which grew out
-// of it).  Registers per thread: the plain kernel fits 3 CTAs of 128 threads per SM (168 registers), the fused-epilogue kernel
-// holds the three update vectors of its site as well and runs 2 CTAs per SM.
+// The four-slot kernel, fp32 only (ND_STENCIL_TILE4; the default is the two-slot kernel, which grew out of it).  Registers per
+// thread: the plain kernel fits 3 CTAs of 128 threads per SM (168 registers), the fused-epilogue kernel holds the three update
+// vectors of its site as well and runs 2 CTAs per SM.  (Its variant with TMA bulk copies - cp.async.bulk, one 512-byte row-plane
+// per lane, 21 requests per warp and slice: 188 / 257 us against 144 / 224 us on 32^3x64 - has been replaced by the tensor-map
+// kernel above.)
 template <int RECON>
 int launch_tile_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                       const void* v2, double s3, const void* v3) {
-    // the prefetch of links and halos: cp.async (LDGSTS, one 16-byte copy per thread and word; the default: 144 / 223 us per
-    // launch on 32^3x64, recon 12) or TMA bulk copies (UBLKCP, one 512-byte row-plane per lane: 21 small requests per warp and
-    // slice keep the SM's TMA unit busier than the data path: 187 / 257 us) - ND_STENCIL_TILE_TMA selects the latter
-    if (ctx->stencil_variant == ND_STENCIL_TILE_TMA) {
-        if (epi) return launch_tile<float, RECON, true, 2, 2, 32, 2, true>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
-        return launch_tile<float, RECON, false, 2, 2, 32, 3, true>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
-    }
-    if (epi) return launch_tile<float, RECON, true, 2, 2, 32, 2, false>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
-    return launch_tile<float, RECON, false, 2, 2, 32, 3, false>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+    if (epi) return launch_tile<float, RECON, true, 2, 2, 32, 2>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile<float, RECON, false, 2, 2, 32, 3>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
 }
 
 }  // namespace
@@ -896,15 +1121,31 @@ static int launch_tile2_shape(nd_ctx* ctx, void* out, const void* in, double m, 
     return launch_tile2<T, RECON, false, MINB, 32>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
 }
 
-// ND_STENCIL_TILE (and auto): the two-slot kernel wilson_Q_tile2_kernel; ND_STENCIL_TILE4 / ND_STENCIL_TILE_TMA (fp32 only): the
-// four-slot kernel wilson_Q_tile_kernel with cp.async / TMA bulk copies
+template <typename T, int RECON, int MINB, int MINB_EPI>
+static int launch_tile3_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
+                              const void* v2, double s3, const void* v3) {
+    if (epi) return launch_tile3<T, RECON, true, MINB_EPI>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile3<T, RECON, false, MINB>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+}
+
+// ND_STENCIL_TILE (and auto): the two-slot kernel wilson_Q_tile2_kernel; ND_STENCIL_TILE_TMA: the same schedule with tensor-map
+// loads, wilson_Q_tile3_kernel (x3 extent 32); ND_STENCIL_TILE4 (fp32, x3 extent 32): the four-slot kernel wilson_Q_tile_kernel
 int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                      const void* v2, double s3, const void* v3) {
+    if (ctx->stencil_variant == ND_STENCIL_TILE_TMA) {
+        if (ctx->prec == 64) {
+            if (ctx->recon == 12) return launch_tile3_shape<double, 12, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+            return launch_tile3_shape<double, 8, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        }
+        if (ctx->recon == 18) return launch_tile3_shape<float, 18, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        if (ctx->recon == 12) return launch_tile3_shape<float, 12, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile3_shape<float, 8, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    }
     if (ctx->prec == 64) {
         if (ctx->recon == 12) return launch_tile2_shape<double, 12, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
         return launch_tile2_shape<double, 8, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
     }
-    if (ctx->stencil_variant == ND_STENCIL_TILE4 || ctx->stencil_variant == ND_STENCIL_TILE_TMA) {
+    if (ctx->stencil_variant == ND_STENCIL_TILE4) {
         if (ctx->recon == 18) return launch_tile_shape<18>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
         if (ctx->recon == 12) return launch_tile_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
         return launch_tile_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);

@@ -75,7 +75,7 @@ def test_spawn_command_and_traffic_table():
         assert t is None or 0.9 * model < t < 1.3 * model                          # a capture, if present, is near the byte model
     assert bench.stencil_kernel_name("site", 8192) == "wilson_Q_hop_kernel" and bench.stencil_kernel_name("site", 1 << 20) == "wilson_Q_kernel"
     assert bench.stencil_kernel_name("tile", 1 << 21) == "wilson_Q_tile2_kernel" and bench.stencil_kernel_name("tile", 1 << 21, 64) == "wilson_Q_tile2_kernel"
-    assert bench.stencil_kernel_name("tile4", 1 << 21) == "wilson_Q_tile_kernel" and bench.stencil_kernel_name("tile_tma", 1 << 21) == "wilson_Q_tile_kernel"
+    assert bench.stencil_kernel_name("tile4", 1 << 21) == "wilson_Q_tile_kernel" and bench.stencil_kernel_name("tile_tma", 1 << 21) == "wilson_Q_tile3_kernel"
 
 
 def test_reference_arm_other_ranks_exit_without_work():

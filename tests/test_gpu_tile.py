@@ -25,7 +25,7 @@ def test_every_variant_matches_the_oracle(dims, bc, recon):
     s0, s1, s2, s3 = 0.37, -1.2, -1.0, 0.81
     ref_epi = s0 * ref + s1 * vecs[0] + s2 * vecs[1] + s3 * vecs[2]
     results = {}
-    for variant in ("site", "tile", "tile4", "tile_tma", "auto"):
+    for variant in ("site", "tile", "tile_tma", "tile4", "auto"):
         ctx.set_stencil_variant(variant)
         ctx.apply_Q(y, x, -1.6)
         got = ctx.unpack_spinor(y)
@@ -35,8 +35,8 @@ def test_every_variant_matches_the_oracle(dims, bc, recon):
         ctx.copy(out, d[1])
         ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])   # out aliases v2, as in the Clenshaw step
         assert rel_l2(ctx.unpack_spinor(out), ref_epi) <= TOL[32], variant
-    # cp.async and TMA prefetch feed the same arithmetic, and so do the two- and the four-slot kernel: bit-identical results
-    assert np.array_equal(results["tile4"], results["tile_tma"]) and np.array_equal(results["tile"], results["tile4"])
+    # cp.async and TMA tensor-map prefetch feed the same arithmetic, and so do the two- and the four-slot kernel: bit-identical
+    assert np.array_equal(results["tile"], results["tile_tma"]) and np.array_equal(results["tile"], results["tile4"])
     assert np.array_equal(results["tile"], results["auto"])       # auto = the tiled kernel
     # worst site against the oracle, not only the norm
     scale = np.abs(ref).max()
@@ -57,7 +57,7 @@ def test_fp64_tiled_kernel_matches_the_oracle(dims, bc, recon):
     s0, s1, s2, s3 = 0.37, -1.2, -1.0, 0.81
     ref_epi = s0 * ref + s1 * vecs[0] + s2 * vecs[1] + s3 * vecs[2]
     results, fused = {}, {}
-    for variant in ("site", "tile", "auto"):
+    for variant in ("site", "tile", "tile_tma", "auto"):
         ctx.set_stencil_variant(variant)
         assert ctx.get_stencil_variant() == ("tile" if variant == "auto" else variant)
         ctx.apply_Q(y, x, -1.6)
@@ -71,6 +71,7 @@ def test_fp64_tiled_kernel_matches_the_oracle(dims, bc, recon):
         assert rel_l2(fused[variant], ref_epi) <= TOL[64], variant
     # auto in fp64: the tiled kernel for the plain stencil, the site-per-thread kernel for the fused-epilogue one
     assert np.array_equal(results["auto"], results["tile"]) and np.array_equal(fused["auto"], fused["site"])
+    assert np.array_equal(results["tile_tma"], results["tile"]) and np.array_equal(fused["tile_tma"], fused["tile"])
     scale = np.abs(ref).max()
     assert np.abs(results["tile"] - ref).max() <= (1e-13 if recon != 8 else 1e-10) * scale
 
@@ -98,9 +99,34 @@ def test_x3_extent_16(dims, bc, prec, recon):
         ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])
         assert rel_l2(ctx.unpack_spinor(out), ref_epi) <= TOL[prec], variant
     import paper_1010_5636_b200 as nd
-    for variant in ("tile4", "tile_tma"):                            # the four-slot kernel exists for x3 extent 32 only
+    for variant in ("tile4", "tile_tma"):                            # the four-slot and tensor-map kernels: x3 extent 32 only
         with pytest.raises(nd.NDError):
             ctx.set_stencil_variant(variant)
+
+
+@pytest.mark.parametrize("prec,dims", [(32, (64, 16, 16, 32)), (64, (64, 16, 16, 32)), (32, (96, 16, 16, 16))])
+def test_tiled_kernel_repeats_bit_for_bit(prec, dims):
+    """The exchange through shared memory and the cp.async slots are race-free by construction (pair barriers, private slots);
+    a race would show up as run-to-run differences: 60 launches of the plain and of the fused stencil, each bit-identical to
+    the first, while the machine is kept busy (several CTAs per SM, many segments)."""
+    import torch
+
+    ctx, U = make_context(dims, prec, 12, -1, "smooth", eps=0.3)
+    ctx.set_stencil_variant("tile")
+    x, y, y0 = ctx.new_spinor(), ctx.new_spinor(), ctx.new_spinor()
+    v = ctx.new_spinor(3)
+    ctx.gaussian(x, 1)
+    for j in range(3):
+        ctx.gaussian(v[j], 2 + j)
+    ctx.apply_Q(y0, x, -1.6)
+    f0 = ctx.new_spinor()
+    ctx.apply_Q_axpbycz(f0, x, -1.6, 0.3, -0.9, v[0], -0.5, v[1], 0.1, v[2])
+    with torch.cuda.stream(ctx.stream):            # the comparisons run on the context's stream, after the launches
+        for _ in range(60):
+            ctx.apply_Q(y, x, -1.6)
+            assert torch.equal(y, y0)
+            ctx.apply_Q_axpbycz(y, x, -1.6, 0.3, -0.9, v[0], -0.5, v[1], 0.1, v[2])
+            assert torch.equal(y, f0)
 
 
 def test_variant_selection_rules():
@@ -114,7 +140,7 @@ def test_variant_selection_rules():
     ctx64, _ = make_context((40, 8, 16, 32), 64, 12)
     assert ctx64.get_stencil_variant() == "tile"
     with pytest.raises(nd.NDError):
-        ctx64.set_stencil_variant("tile_tma")                        # the bulk-copy variant exists in fp32 only
+        ctx64.set_stencil_variant("tile4")                           # the four-slot kernel exists in fp32 only
     ctx64b, _ = make_context((40, 2, 16, 32), 64, 12)                # fp64 tiles need x1 / x2 extents >= 4
     with pytest.raises(nd.NDError):
         ctx64b.set_stencil_variant("tile")
