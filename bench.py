@@ -492,7 +492,7 @@ def run_b200(args):
     decompose = world > 1 and not args.replicas
     if decompose:
         # domain decomposition: this rank's time-slices of the one global lattice (nd_shard_layout), faces over NCCL
-        from paper_1010_5636_b200.dist import TorchDistComm
+        from paper_1010_5636_b200.dist import PeerComm, TorchDistComm
 
         tb, tl, _, _ = nd.shard_layout(gdims[0], world, rank)
         dims = (tl,) + tuple(gdims[1:])
@@ -507,7 +507,8 @@ def run_b200(args):
         return
     ctx = nd.Context(dims, prec=prec, recon=recon, bc_time=-1, device=local)
     ctx.set_gauge(Uloc.astype(np.complex64) if prec == 32 else Uloc)
-    comm = TorchDistComm(ctx) if decompose else None      # from here on every call acts on the global lattice
+    # from here on every call acts on the global lattice; --p2p: faces stored by the pack kernel into the neighbours' windows
+    comm = (PeerComm(ctx) if args.p2p else TorchDistComm(ctx)) if decompose else None
     V = ctx.V                                             # sites of this rank
     c, delta = nd.cheb_coeffs(n, args.eps)
     ctx.set_sign_poly(c, args.eps, QNORM, M_KERNEL)
@@ -628,7 +629,8 @@ def run_b200(args):
                    "lattice": args.lattice, "sites": V_global, "sites_per_gpu": V, "recon": recon, "degree": n, "eps": args.eps,
                    "delta": delta, "lowmodes": l, "lowmodes_kind": modes_kind, "stencil_variant": headline_variant,
                    "parallelism": (f"domain decomposition along x0 over {world} GPUs ({gdims[0] // world} slices each), "
-                                   f"half-spinor faces over NCCL" if decompose else f"replicas x{world}"),
+                                   f"half-spinor faces {'stored peer-to-peer into symmetric memory' if args.p2p else 'over NCCL'}"
+                                   if decompose else f"replicas x{world}"),
                    "l2_policy": "inputs larger than L2 (links + vectors >= 1.4 GB fp32), no flush needed"},
         "dn_applies_per_s": (1 if decompose else world) * args.steps / (ms * 1e-3),
         "q_stencils_per_s": (1 if decompose else world) * args.steps * stencils / (ms * 1e-3),
@@ -699,6 +701,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--q-only", action="store_true", help="time only the Q stencil of --prec / --recon on --lattice (plain and fused epilogue)")
     ap.add_argument("--variant", default=None, choices=["site", "tile", "tile_tma", "tile4"], help="with --q-only: force a stencil variant")
+    ap.add_argument("--p2p", action="store_true", help="--gpus N: peer-to-peer face exchange (dist.PeerComm) instead of NCCL send/recv")
     ap.add_argument("--replicas", action="store_true", help="--gpus N as N independent lattices (weak scaling) instead of the domain decomposition")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup

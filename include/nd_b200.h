@@ -263,6 +263,17 @@ ND_API int nd_shard_layout(int T, int nranks, int rank, int* t_begin, int* t_loc
 ND_API int nd_set_sharding(nd_ctx* ctx, int rank, int nranks, nd_exchange_start_fn start, nd_exchange_wait_fn wait,
                            nd_allreduce_fn allreduce, void* user);
 ND_API size_t nd_halo_bytes(const nd_ctx* ctx);   /* bytes of one face: (V_local / T_local) * 12 reals */
+/* Peer-to-peer mode of the face exchange: instead of packing into the context's send buffers and handing them to the `start`
+ * callback, the pack kernel STORES the two faces directly into the neighbours' receive windows - the compute kernel's stores
+ * are the transfer (over NVLink 5 / NVSwitch when the windows are peer-mapped device memory of the neighbouring GPUs, e.g. a
+ * symmetric-memory allocation; paper_1010_5636_b200/dist.py: PeerComm).  A window is 4 * nd_halo_bytes(ctx) bytes of device
+ * memory, caller-owned, laid out [parity 2][from_prev, from_next][nd_halo_bytes]: consecutive stencil applications alternate
+ * between the two halves, so a rank may write the faces of application n+1 into a neighbour that is still consuming those of
+ * application n.  recv_own = this rank's window, recv_of_next / recv_of_prev = the windows of the next / previous rank (the same
+ * pointer twice when nranks = 2).  `start` is not called in this mode (it may be NULL in nd_set_sharding); `wait` must be a
+ * barrier over the ranks ordered with the context's stream: when the stream passes it, every rank's pack kernel of this
+ * application has completed and its stores are visible.  All three NULL: back to the callback transfers. */
+ND_API int nd_set_halo_peers(nd_ctx* ctx, void* recv_own, void* recv_of_next, void* recv_of_prev);
 ND_API int nd_halo_buffers(nd_ctx* ctx, void** send_next, void** send_prev, void** recv_prev, void** recv_next);
 
 /* ------------------------------------------------------------------------------------------------ BLAS-1

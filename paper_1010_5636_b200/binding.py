@@ -38,6 +38,7 @@ SIGNATURES = {
     "nd_shard_layout": (_c_int, [_c_int, _c_int, _c_int, ctypes.POINTER(_c_int), ctypes.POINTER(_c_int), ctypes.POINTER(_c_int),
                                  ctypes.POINTER(_c_int)]),
     "nd_set_sharding": (_c_int, [_c_vp, _c_int, _c_int, _c_vp, _c_vp, _c_vp, _c_vp]),
+    "nd_set_halo_peers": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp]),
     "nd_halo_bytes": (_c_sz, [_c_vp]),
     "nd_halo_buffers": (_c_int, [_c_vp, ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp)]),
     "nd_set_stencil_variant": (_c_int, [_c_vp, _c_int]),
@@ -280,12 +281,19 @@ class Context:
             return call
 
         if nranks > 1:
-            self._cb = (EXCHANGE_START_FN(guard(start)), EXCHANGE_WAIT_FN(guard(wait)), ALLREDUCE_FN(guard(allreduce)))
-            self._chk(self.lib.nd_set_sharding(self._h, int(rank), int(nranks), ctypes.cast(self._cb[0], _c_vp),
+            self._cb = (EXCHANGE_START_FN(guard(start)) if start is not None else None, EXCHANGE_WAIT_FN(guard(wait)),
+                        ALLREDUCE_FN(guard(allreduce)))
+            self._chk(self.lib.nd_set_sharding(self._h, int(rank), int(nranks),
+                                               ctypes.cast(self._cb[0], _c_vp) if start is not None else None,
                                                ctypes.cast(self._cb[1], _c_vp), ctypes.cast(self._cb[2], _c_vp), None))
         else:
             self._chk(self.lib.nd_set_sharding(self._h, 0, 1, None, None, None, None))
             self._cb = None
+
+    def set_halo_peers(self, recv_own, recv_of_next, recv_of_prev):
+        """Peer-to-peer face exchange (nd_set_halo_peers): raw device pointers (ints) of the three receive windows of
+        4 * halo_bytes() bytes each, or three None for the callback transfers."""
+        self._chk(self.lib.nd_set_halo_peers(self._h, recv_own, recv_of_next, recv_of_prev))
 
     def halo_bytes(self):
         return int(self.lib.nd_halo_bytes(self._h))

@@ -83,6 +83,8 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     ctx->shard_n = 1;
     ctx->in_shard_call = false;
     for (int i = 0; i < 4; i++) ctx->halo[i] = nullptr;
+    ctx->peer_own = ctx->peer_next = ctx->peer_prev = nullptr;
+    ctx->halo_parity = 0;
     ctx->exchange_start = nullptr;
     ctx->exchange_wait = nullptr;
     ctx->allreduce = nullptr;

@@ -68,6 +68,12 @@ struct nd_ctx {
     int shard_rank, shard_n;
     bool in_shard_call;         // the local stencil of a sharded application is being enqueued
     void* halo[4];              // send_next, send_prev, recv_prev, recv_next: half-spinor faces (nd_halo_bytes each)
+    // peer-to-peer mode (nd_set_halo_peers): faces are STORED by halo_pack straight into the neighbours' receive windows
+    // [parity 2][from_prev, from_next][nd_halo_bytes]; nullptr = callback transfers through halo[0..3]
+    void* peer_own;             // this rank's receive window
+    void* peer_next;            // the next rank's window (its from_prev faces are written by this rank)
+    void* peer_prev;            // the previous rank's window (its from_next faces)
+    int halo_parity;
     nd_exchange_start_fn exchange_start;
     nd_exchange_wait_fn exchange_wait;
     nd_allreduce_fn allreduce;

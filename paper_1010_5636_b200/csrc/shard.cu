@@ -116,7 +116,16 @@ int halo_pack_t(nd_ctx* ctx, const void* in) {
     const dim3 grid((unsigned)((S0 + 127) / 128), 2, 1);
     const T pn = (ctx->shard_rank == ctx->shard_n - 1) ? T(ctx->bc) : T(1);
     const T pp = (ctx->shard_rank == 0) ? T(ctx->bc) : T(1);
-    halo_pack_kernel<T, RECON><<<grid, 128, 0, ctx->stream>>>((Vec*)ctx->halo[0], (Vec*)ctx->halo[1], (const Vec*)in, (const LVec*)ctx->gauge,
+    // destinations: the own send buffers (the caller's callbacks move them), or - peer-to-peer mode - the neighbours' receive
+    // windows themselves: the stores of this kernel ARE the transfer (over NVLink when the windows are peer-mapped)
+    Vec* to_next = (Vec*)ctx->halo[0];
+    Vec* to_prev = (Vec*)ctx->halo[1];
+    if (ctx->peer_own) {
+        const size_t hb = nd_halo_bytes(ctx);
+        to_next = (Vec*)((char*)ctx->peer_next + (size_t)(2 * ctx->halo_parity + 0) * hb);   // the next rank's from_prev face
+        to_prev = (Vec*)((char*)ctx->peer_prev + (size_t)(2 * ctx->halo_parity + 1) * hb);   // the previous rank's from_next face
+    }
+    halo_pack_kernel<T, RECON><<<grid, 128, 0, ctx->stream>>>(to_next, to_prev, (const Vec*)in, (const LVec*)ctx->gauge,
                                                                 ctx->V, S0, ctx->dims[0], pn, pp);
     ND_LAUNCHED(ctx);
     return ND_OK;
@@ -127,8 +136,15 @@ int halo_apply_t(nd_ctx* ctx, void* out, double s0) {
     using LVec = typename LinkLayout<T, RECON>::LVec;
     const long long S0 = ctx->V / ctx->dims[0];
     const dim3 grid((unsigned)((S0 + 127) / 128), 2, 1);
-    halo_apply_kernel<T, RECON><<<grid, 128, 0, ctx->stream>>>((Vec*)out, (const Vec*)ctx->halo[2], (const Vec*)ctx->halo[3],
-                                                                 (const LVec*)ctx->gauge, ctx->V, S0, ctx->dims[0], T(s0));
+    const Vec* from_prev = (const Vec*)ctx->halo[2];
+    const Vec* from_next = (const Vec*)ctx->halo[3];
+    if (ctx->peer_own) {
+        const size_t hb = nd_halo_bytes(ctx);
+        from_prev = (const Vec*)((const char*)ctx->peer_own + (size_t)(2 * ctx->halo_parity + 0) * hb);
+        from_next = (const Vec*)((const char*)ctx->peer_own + (size_t)(2 * ctx->halo_parity + 1) * hb);
+    }
+    halo_apply_kernel<T, RECON><<<grid, 128, 0, ctx->stream>>>((Vec*)out, from_prev, from_next, (const LVec*)ctx->gauge, ctx->V, S0,
+                                                                 ctx->dims[0], T(s0));
     ND_LAUNCHED(ctx);
     return ND_OK;
 }
@@ -168,7 +184,7 @@ extern "C" int nd_set_sharding(nd_ctx* ctx, int rank, int nranks, nd_exchange_st
                                nd_allreduce_fn allreduce, void* user) {
     if (!ctx) return ND_ERR_BAD_ARG;
     if (nranks < 1 || rank < 0 || rank >= nranks) return nd_fail(ctx, ND_ERR_BAD_ARG, "set_sharding: bad rank %d of %d", rank, nranks);
-    if (nranks > 1 && (!start || !wait || !allreduce)) return nd_fail(ctx, ND_ERR_BAD_ARG, "set_sharding: callbacks missing");
+    if (nranks > 1 && (!wait || !allreduce)) return nd_fail(ctx, ND_ERR_BAD_ARG, "set_sharding: callbacks missing");
     ND_CUDA(ctx, cudaSetDevice(ctx->device));
     ndi_drop_graphs(ctx);
     for (int i = 0; i < 4; i++) {
@@ -181,8 +197,25 @@ extern "C" int nd_set_sharding(nd_ctx* ctx, int rank, int nranks, nd_exchange_st
     ctx->exchange_wait = wait;
     ctx->allreduce = allreduce;
     ctx->comm_user = user;
+    ctx->peer_own = ctx->peer_next = ctx->peer_prev = nullptr;
+    ctx->halo_parity = 0;
     if (nranks > 1)
         for (int i = 0; i < 4; i++) ND_CUDA(ctx, cudaMalloc(&ctx->halo[i], nd_halo_bytes(ctx)));
+    return ND_OK;
+}
+
+extern "C" int nd_set_halo_peers(nd_ctx* ctx, void* recv_own, void* recv_of_next, void* recv_of_prev) {
+    if (!ctx) return ND_ERR_BAD_ARG;
+    if (ctx->shard_n <= 1) return nd_fail(ctx, ND_ERR_BAD_STATE, "set_halo_peers: the context is not sharded (nd_set_sharding first)");
+    const bool all = recv_own && recv_of_next && recv_of_prev, none = !recv_own && !recv_of_next && !recv_of_prev;
+    if (!all && !none) return nd_fail(ctx, ND_ERR_BAD_ARG, "set_halo_peers: give all three windows or none");
+    if (none && !ctx->exchange_start) return nd_fail(ctx, ND_ERR_BAD_STATE, "set_halo_peers: no exchange-start callback to fall back to");
+    if (all && ((((size_t)recv_own | (size_t)recv_of_next | (size_t)recv_of_prev) & 15) != 0 || (nd_halo_bytes(ctx) & 15) != 0))
+        return nd_fail(ctx, ND_ERR_BAD_ARG, "set_halo_peers: windows must be 16-byte aligned");
+    ctx->peer_own = recv_own;
+    ctx->peer_next = recv_of_next;
+    ctx->peer_prev = recv_of_prev;
+    ctx->halo_parity = 0;
     return ND_OK;
 }
 

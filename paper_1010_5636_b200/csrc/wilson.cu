@@ -302,8 +302,11 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
             const size_t o = (size_t)j * sb;
             int rc = ndi_halo_pack(ctx, (const char*)in + o);
             if (rc != ND_OK) return rc;
-            if (ctx->exchange_start(ctx->comm_user, ctx->halo[0], ctx->halo[1], ctx->halo[2], ctx->halo[3], nd_halo_bytes(ctx)) != 0)
-                return nd_fail(ctx, ND_ERR_CUDA, "sharding: the exchange-start callback failed");
+            if (!ctx->peer_own) {   // (peer-to-peer mode: the pack kernel has already stored the faces where they belong)
+                if (!ctx->exchange_start) return nd_fail(ctx, ND_ERR_BAD_STATE, "sharding: neither an exchange-start callback nor peer windows");
+                if (ctx->exchange_start(ctx->comm_user, ctx->halo[0], ctx->halo[1], ctx->halo[2], ctx->halo[3], nd_halo_bytes(ctx)) != 0)
+                    return nd_fail(ctx, ND_ERR_CUDA, "sharding: the exchange-start callback failed");
+            }
             ctx->in_shard_call = true;
             const int saved_bc = ctx->bc;
             ctx->bc = 0;   // phase of the hops across the local time boundary: they come from the neighbours instead
@@ -315,6 +318,7 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
             if (ctx->exchange_wait(ctx->comm_user) != 0) return nd_fail(ctx, ND_ERR_CUDA, "sharding: the exchange-wait callback failed");
             rc = ndi_halo_apply(ctx, (char*)out + o, epi ? s0 : 1.0);
             if (rc != ND_OK) return rc;
+            ctx->halo_parity ^= 1;   // the next application uses the other half of the receive windows
         }
         return ND_OK;
     }

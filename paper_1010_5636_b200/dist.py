@@ -49,3 +49,36 @@ class TorchDistComm:
         t = self.ctx.wrap_device_memory(d_buf, 8 * n, torch.float64)
         with torch.cuda.stream(self.ctx.stream):
             dist.all_reduce(t, group=self.group)
+
+
+class PeerComm(TorchDistComm):
+    """Peer-to-peer face exchange (nd_set_halo_peers): the receive windows live in a symmetric-memory allocation that every rank
+    of the node maps (torch.distributed._symmetric_memory: CUDA IPC / fabric handles over NVLink), the library's pack kernel
+    stores each face straight into the neighbour's window, and `wait` is the allocation's device-side barrier enqueued on the
+    context's stream - no NCCL call on the stencil's path; reductions still go through all_reduce.  One node only."""
+
+    def __init__(self, ctx, group=None):
+        super().__init__(ctx, group)
+        if self.world > 1:
+            import torch.distributed._symmetric_memory as symm_mem
+
+            g = group if group is not None else dist.group.WORLD
+            with torch.cuda.stream(ctx.stream):
+                self.window = symm_mem.empty(4 * ctx.halo_bytes(), dtype=torch.uint8, device=ctx.torch_device)
+                self.window.zero_()
+            self.handle = symm_mem.rendezvous(self.window, g)
+            ptrs = window_pointers(list(self.handle.buffer_ptrs), self.rank, self.world)
+            ctx.set_halo_peers(*ptrs)
+
+    def start(self, *a):                                   # never called in peer-to-peer mode
+        raise RuntimeError("PeerComm: the exchange-start callback must not be called while peer windows are set")
+
+    def wait(self):
+        with torch.cuda.stream(self.ctx.stream):
+            self.handle.barrier()
+
+
+def window_pointers(all_windows, rank, world):
+    """(own, next rank's, previous rank's) receive window out of the per-rank list of a symmetric allocation."""
+    prev, nxt = ring_neighbours(rank, world)
+    return all_windows[rank], all_windows[nxt], all_windows[prev]

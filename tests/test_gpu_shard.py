@@ -21,7 +21,7 @@ pytestmark = pytest.mark.gpu
 class Emulation:
     """R ranks in one process: thread r drives context r; faces and reductions meet at barriers."""
 
-    def __init__(self, dims, R, prec, recon, bc, U):
+    def __init__(self, dims, R, prec, recon, bc, U, peers=False):
         import torch
 
         import paper_1010_5636_b200 as nd
@@ -40,6 +40,16 @@ class Emulation:
         for r, c in enumerate(self.ctx):
             c.set_sharding(r, R, self._start(r), self._wait(r), self._allreduce(r))
         self.bufs = [[c.wrap_device_memory(p, c.halo_bytes(), c.real_dtype) for p in c.halo_buffers()] for c in self.ctx]
+        if peers:
+            # peer-to-peer mode (nd_set_halo_peers): one receive window per rank, the neighbours' pack kernels store into it;
+            # the start callback must never run, the wait callback is a barrier over the ranks after a stream synchronise
+            from paper_1010_5636_b200.dist import window_pointers
+
+            self.windows = [torch.full((4 * c.halo_bytes(),), 0xFF, dtype=torch.uint8, device=c.torch_device) for c in self.ctx]   # NaN bits
+            torch.cuda.synchronize()
+            for r, c in enumerate(self.ctx):
+                c.set_sharding(r, R, None, self._wait(r), self._allreduce(r))
+                c.set_halo_peers(*window_pointers([w.data_ptr() for w in self.windows], r, R))
 
     def _start(self, r):
         def start(send_next, send_prev, recv_prev, recv_next, nbytes):
@@ -95,11 +105,12 @@ class Emulation:
         return [np.ascontiguousarray(field[r * self.tl:(r + 1) * self.tl]) for r in range(self.R)]
 
 
+@pytest.mark.parametrize("peers", [False, True])
 @pytest.mark.parametrize("dims,R,prec,recon,bc", [((16, 4, 4, 8), 2, 64, 12, -1), ((16, 4, 4, 8), 4, 64, 8, -1), ((8, 4, 6, 4), 2, 32, 18, +1),
                                                    ((80, 8, 16, 32), 2, 32, 12, -1), ((32, 8, 8, 16), 2, 32, 12, -1)])
-def test_sharded_Q_matches_oracle(dims, R, prec, recon, bc):
+def test_sharded_Q_matches_oracle(dims, R, prec, recon, bc, peers):
     U = round_to(gauge_field(dims, "smooth", eps=0.3), prec)
-    em = Emulation(dims, R, prec, recon, bc, U)
+    em = Emulation(dims, R, prec, recon, bc, U, peers=peers)
     psi = round_to(gaussian_spinor(dims), prec)
     v = [round_to(gaussian_spinor(dims, seed=30 + i), prec) for i in range(2)]
     ref = wilson_c.apply_Q(psi, U, -1.6, bc)
@@ -127,10 +138,11 @@ def test_sharded_Q_matches_oracle(dims, R, prec, recon, bc):
         assert res[0][4] == "tile"                                          # the tiled kernel ran the local lattices
 
 
-def test_sharded_DN_and_eigensolver():
+@pytest.mark.parametrize("peers", [False, True])
+def test_sharded_DN_and_eigensolver(peers):
     dims, R, prec = (16, 4, 4, 8), 2, 64
     U = gauge_field(dims, "smooth", eps=0.3)
-    em = Emulation(dims, R, prec, 12, -1, U)
+    em = Emulation(dims, R, prec, 12, -1, U, peers=peers)
     Q = wilson_c.make_Q(U, M, -1)
     eta = gaussian_spinor(dims)
     nu, Us = low_space(Q, eta.shape, 5, cut=1.0, degree=8)
@@ -172,6 +184,9 @@ def test_sharding_argument_checks():
     import paper_1010_5636_b200 as nd
 
     ctx = nd.Context((4, 4, 4, 4), prec=64, recon=12)
+    with pytest.raises(nd.NDError) as e:
+        ctx.set_halo_peers(None, None, None)                                 # peer windows need a sharded context
+    assert e.value.code == -2
     with pytest.raises(nd.NDError):
         ctx.lib.nd_set_sharding(ctx._h, 2, 2, None, None, None, None) and None
         ctx._chk(ctx.lib.nd_set_sharding(ctx._h, 2, 2, None, None, None, None))

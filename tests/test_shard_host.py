@@ -12,6 +12,15 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
+def test_window_pointers_of_the_peer_to_peer_exchange():
+    from paper_1010_5636_b200.dist import ring_neighbours, window_pointers
+
+    w = [100, 200, 300, 400]
+    assert window_pointers(w, 0, 4) == (100, 200, 400) and window_pointers(w, 3, 4) == (400, 100, 300)
+    assert window_pointers(w[:2], 1, 2) == (200, 100, 100)                   # two ranks: previous and next are the same peer
+    assert ring_neighbours(0, 1) == (0, 0)
+
+
 def test_shard_layout():
     import paper_1010_5636_b200 as nd
 
