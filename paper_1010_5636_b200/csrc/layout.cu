@@ -127,7 +127,7 @@ __global__ void convert_spinor_kernel(typename Prec<Td>::Vec* __restrict__ dst, 
 // --------------------------------------------------------------------------------------------------- links
 // the statistics are non-negative doubles: their bit patterns order like the values.  A NaN must not be lost on the way
 // (fmax/fmin drop NaN operands), so every candidate is first mapped NaN -> +inf for the maxima and NaN -> 0 for the minimum.
-__device__ __forceinline__ double nan_to(double x, double v) { return (x == x) ? x : v; }
+template <typename C> __device__ __forceinline__ C nan_to(C x, C v) { return (x == x) ? x : v; }
 __device__ __forceinline__ void atomic_max_nonneg(double* addr, double v) {
     atomicMax(reinterpret_cast<unsigned long long*>(addr), (unsigned long long)__double_as_longlong(v));
 }
@@ -153,26 +153,27 @@ __global__ void __launch_bounds__(LAYOUT_THREADS) compress_gauge_kernel(typename
     const int t = threadIdx.x;
     const bool valid = t < ns;
     const int tr = valid ? t : 0;   // keep the whole warp alive for the shuffles below; the store is predicated
-    cx<double> U[3][3];
+    // checks in the precision of the links as given (C): fp32 input is judged against 2e-5, fp32 arithmetic resolves 1e-7
+    using C = Tin;
+    cx<C> U[3][3];
 #pragma unroll
     for (int a = 0; a < 3; a++)
 #pragma unroll
-        for (int b = 0; b < 3; b++) U[a][b] = {(double)tile[tr * ST + 2 * (3 * a + b)], (double)tile[tr * ST + 2 * (3 * a + b) + 1]};
-    // checks in fp64 on the values as given
-    double dev = 0.0;
+        for (int b = 0; b < 3; b++) U[a][b] = {tile[tr * ST + 2 * (3 * a + b)], tile[tr * ST + 2 * (3 * a + b) + 1]};
+    C dev_c = C(0);
 #pragma unroll
     for (int a = 0; a < 3; a++)
 #pragma unroll
         for (int b = 0; b < 3; b++) {
-            cx<double> acc = {a == b ? -1.0 : 0.0, 0.0};
+            cx<C> acc = {a == b ? C(-1) : C(0), C(0)};
 #pragma unroll
             for (int k = 0; k < 3; k++) cfma_cj(acc, U[k][a], U[k][b]);
-            dev = fmax(dev, fmax(nan_to(fabs(acc.re), INFINITY), nan_to(fabs(acc.im), INFINITY)));
+            dev_c = fmax(dev_c, fmax(nan_to(fabs(acc.re), C(INFINITY)), nan_to(fabs(acc.im), C(INFINITY))));
         }
-    cx<double> det = U[0][0] * (U[1][1] * U[2][2] - U[1][2] * U[2][1]) - U[0][1] * (U[1][0] * U[2][2] - U[1][2] * U[2][0]) +
+    cx<C> det = U[0][0] * (U[1][1] * U[2][2] - U[1][2] * U[2][1]) - U[0][1] * (U[1][0] * U[2][2] - U[1][2] * U[2][0]) +
                      U[0][2] * (U[1][0] * U[2][1] - U[1][1] * U[2][0]);
-    double ddev = fmax(nan_to(fabs(det.re - 1.0), INFINITY), nan_to(fabs(det.im), INFINITY));
-    double N = nan_to(U[0][1].re * U[0][1].re + U[0][1].im * U[0][1].im + U[0][2].re * U[0][2].re + U[0][2].im * U[0][2].im, 0.0);
+    C ddev_c = fmax(nan_to(fabs(det.re - C(1)), C(INFINITY)), nan_to(fabs(det.im), C(INFINITY)));
+    C N_c = nan_to(U[0][1].re * U[0][1].re + U[0][1].im * U[0][1].im + U[0][2].re * U[0][2].re + U[0][2].im * U[0][2].im, C(0));
     T r[LL::NL * W];
     if (RECON == 18) {
 #pragma unroll
@@ -189,8 +190,8 @@ __global__ void __launch_bounds__(LAYOUT_THREADS) compress_gauge_kernel(typename
         r[2] = (T)U[0][2].re; r[3] = (T)U[0][2].im;
         r[4] = (T)U[1][0].re; r[5] = (T)U[1][0].im;
         // the two phases are stored as tan(theta/4) in [-1, 1]: rebuilt with one reciprocal, no sincos (nd_su3.cuh)
-        r[6] = (T)tan(0.25 * atan2(U[0][0].im, U[0][0].re));
-        r[7] = (T)tan(0.25 * atan2(U[2][0].im, U[2][0].re));
+        r[6] = (T)tan(0.25 * atan2((double)U[0][0].im, (double)U[0][0].re));
+        r[7] = (T)tan(0.25 * atan2((double)U[2][0].im, (double)U[2][0].re));
     }
     LVec words[LL::NL];
 #pragma unroll
@@ -200,7 +201,7 @@ __global__ void __launch_bounds__(LAYOUT_THREADS) compress_gauge_kernel(typename
         for (int k = 0; k < W; k++) wr[k] = r[p * W + k];
     }
     // what the stencil will see: rebuild the link from the stored words with the stencil's own routine and compare
-    double rerr = 0.0;
+    C rerr_c = C(0);
     {
         cx<T> R[3][3];
         reconstruct_link<T, RECON>(words, R);
@@ -208,10 +209,11 @@ __global__ void __launch_bounds__(LAYOUT_THREADS) compress_gauge_kernel(typename
         for (int a = 0; a < 3; a++)
 #pragma unroll
             for (int b = 0; b < 3; b++)
-                rerr = fmax(rerr, fmax(nan_to(fabs((double)R[a][b].re - U[a][b].re), INFINITY),
-                                       nan_to(fabs((double)R[a][b].im - U[a][b].im), INFINITY)));
+                rerr_c = fmax(rerr_c, fmax(nan_to(fabs((C)R[a][b].re - U[a][b].re), C(INFINITY)),
+                                       nan_to(fabs((C)R[a][b].im - U[a][b].im), C(INFINITY))));
     }
-    // warp-level reduce before the atomics
+    // warp-level reduce before the atomics (statistics in fp64 from here on)
+    double dev = dev_c, ddev = ddev_c, rerr = rerr_c, N = N_c;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         dev = fmax(dev, __shfl_xor_sync(0xffffffffu, dev, o));
