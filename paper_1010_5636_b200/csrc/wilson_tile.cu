@@ -317,7 +317,7 @@ __global__ void __launch_bounds__(B1* B2* L3, MINB)
     constexpr int K2 = PairSync<B1, B2, L3>::value ? 0 : 2;
     constexpr int ROW1 = B2 * L3;   // slot distance of x1 neighbours
     constexpr int ROW2 = L3;        // slot distance of x2 neighbours
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     Vec* xbuf = reinterpret_cast<Vec*>(smem_raw);                                  // exchange: [NK kinds][NW][NT]
     LVec* lnk = reinterpret_cast<LVec*>(smem_raw + (size_t)NK * NW * NT * sizeof(Vec));   // links: [4 mu][NL][NT]
     unsigned char* hal = smem_raw + (size_t)NK * NW * NT * sizeof(Vec) + (size_t)4 * LL::NL * NT * sizeof(LVec);   // halo slot
@@ -520,7 +520,7 @@ __global__ void __launch_bounds__(128, MINB)
     constexpr int HLN = 3 * 32;                // halo link entries: the three rows of a tile that have a backward face
     constexpr int NW = HalfWords<T>::NW, NV = Prec<T>::NV;
     constexpr int ROW1 = 2 * L3, ROW2 = L3;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     unsigned char* sp = smem_raw;
     Vec* xbuf = reinterpret_cast<Vec*>(sp);   sp += (size_t)2 * NW * NT * sizeof(Vec);        // exchange: [2 kinds][NW][NT]
     LVec* lnkA = reinterpret_cast<LVec*>(sp); sp += (size_t)LL::NL * NT * sizeof(LVec);       // link slot A: x1, then x2
