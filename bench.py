@@ -17,6 +17,7 @@ roofline = the dominant kernel (the Q stencil), timed alone with CUDA events on 
            (median of 5 batches, clocks sampled meanwhile), against the measured HBM copy peak of MEASURED_PEAKS.json;
            `q_kernel` holds every precision x recon variant and, for fp32, the stencil variants against each other.
 layout   = a1 alone: pack / unpack / link compression, GB/s over AoS + SoA bytes.
+projection = a7 alone: block dot and block axpy over l vectors (32^3x64 l = 8; 16^3x32 l = 50), GB/s over the compulsory bytes.
 configs  = the other timed BASELINE.json configurations, driver-run in the same line: index 1 (1000 back-to-back Q on
            16^3x32, fp32 + fp64 x recon 12 / 8), index 3 (D_N on 8^3x16, fp64, about 20 modes from the library's
            eigen-solver) and index 4 (D_N on 16^3x32, fp32, about 50 modes, degree 200, eigen-solve timed).
@@ -270,7 +271,7 @@ def measure_q_kernel(torch, nd, dims, lattice, U64, prec, recon, peak, variants=
                 ctx.gaussian(v[j], 77 + j)
             msf, _ = median_of_batches(torch, ctx, lambda: ctx.apply_Q_axpbycz(v[1], x, M_KERNEL, 0.05, -0.9, v[0], -0.5, v[1], 0.01, v[2]), reps)
             gbf = q_bytes_per_site(prec, recon, 3) * V / (msf * 1e-3) / 1e9
-            out["fused_epilogue"] = {"kernel": stencil_kernel_name("site" if (prec == 64 and var is None) else name, V, prec),
+            out["fused_epilogue"] = {"kernel": stencil_kernel_name("site" if (prec == 64 and recon != 12 and var is None) else name, V, prec),
                                      "us_per_launch": msf * 1e3, "bytes_per_site": q_bytes_per_site(prec, recon, 3),
                                      "achieved_gbs": gbf, "frac_of_measured_peak": gbf / peak, "frac_of_8TBs": gbf / 8000.0}
             del v
@@ -313,6 +314,35 @@ def measure_layout(torch, nd, dims, U64, prec, peak):
     res["prec"] = prec
     ctx.close()
     del aos, back, Ud, soa
+    torch.cuda.empty_cache()
+    return res
+
+
+def measure_projection(torch, nd, lattice, l, prec, peak):
+    """a7 alone: block dot (V^dagger x, l vectors) and block axpy (y += V a) through the `_dev` calls (no host synchronisation),
+    GB/s over the compulsory bytes ((l + 1) resp. (l + 2) spinor streams)."""
+    from lattice_inputs import parse_lattice
+
+    dims = parse_lattice(lattice)
+    ctx = nd.Context(dims, prec=prec, recon=12, bc_time=-1)
+    V, b = ctx.V, prec // 8
+    Vb, x = ctx.new_spinor(l), ctx.new_spinor()
+    for k in range(l):
+        ctx.gaussian(Vb[k], 300 + k)
+    ctx.gaussian(x, 299)
+    with torch.cuda.stream(ctx.stream):
+        c = torch.zeros(2 * l, dtype=torch.float64, device=ctx.torch_device)
+        a = torch.full((2 * l,), 1e-3, dtype=torch.float64, device=ctx.torch_device)
+    reps = 20 if V * l < (1 << 26) else 5
+    ms_dot, _ = median_of_batches(torch, ctx, lambda: ctx.block_dot_dev(Vb, x, c), reps)
+    ms_axpy, _ = median_of_batches(torch, ctx, lambda: ctx.block_axpy_dev(a, Vb, x), reps)
+    res = {"lattice": lattice, "prec": prec, "l": l, "block_bytes": l * 24 * b * V,
+           "block_dot": {"us": ms_dot * 1e3, "gbs": (l + 1) * 24 * b * V / (ms_dot * 1e-3) / 1e9},
+           "block_axpy": {"us": ms_axpy * 1e3, "gbs": (l + 2) * 24 * b * V / (ms_axpy * 1e-3) / 1e9}}
+    for k in ("block_dot", "block_axpy"):
+        res[k]["frac_of_measured_peak"] = res[k]["gbs"] / peak
+    ctx.close()
+    del Vb, x, c, a
     torch.cuda.empty_cache()
     return res
 
@@ -651,9 +681,11 @@ def run_b200(args):
                 "us_per_launch": main["us_per_launch"], "timing": "median of 5 batches of 20 launches, CUDA events on the launch stream",
                 "frac_of_8TBs_nominal": main["achieved_gbs"] / 8000.0, "clocks": q_clocks,
                 "traffic_source": "profiles/q_kernel_dram_traffic.csv (ncu --set full of this kernel on this lattice; null = no capture)"}
-    layout, configs, cpu = None, [], None
+    layout, projection, configs, cpu = None, None, [], None
     if not args.quick:
         layout = {f"f{p}": measure_layout(torch, nd, dims, U64, p, peak) for p in (32, 64)}
+        projection = [measure_projection(torch, nd, "32^3x64", 8, 32, peak), measure_projection(torch, nd, "16^3x32", 50, 32, peak),
+                      measure_projection(torch, nd, "16^3x32", 50, 64, peak)]
         configs.append(q_config(torch, nd))
         configs.append(dn_config(torch, nd, 3, "8^3x16", 64, 0.3, (16, 24), 8, 100, 60, 1e-6, nrhs=8))
         configs.append(dn_config(torch, nd, 4, "16^3x32", 32, 0.25, (44, 56), 12, 200, 160, 1e-2, nrhs=4))
@@ -690,6 +722,7 @@ def run_b200(args):
         "roofline": roofline,
         "q_kernel": qk,
         "layout": layout,
+        "projection": projection,
         "configs": configs,
         "cpu_baseline": cpu,
     }

@@ -73,8 +73,8 @@ ND_API size_t nd_gauge_bytes(const nd_ctx* ctx);        /* bytes of the compress
 /* Which kernel applies the stencil (csrc/wilson.cu, csrc/wilson_tile.cu).  ND_STENCIL_AUTO (default)
  * picks the fastest one measured for the context and call: the tiled marching kernel (neighbour exchange through shared memory,
  * cp.async prefetch of links, halos and the next spinor) on lattices it supports - x3 extent 32 or 16, even x1 / x2 extents >= 4
- * (x3 extent 16: x2 extent divisible by 4), at least 8 slices of 128 sites per SM, in fp64 recon 12 / 8 and the plain stencil
- * only - and the site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The other values force one kernel for every
+ * (x3 extent 16: x2 extent divisible by 4), at least 8 slices of 128 sites per SM, in fp64 recon 12 / 8 (recon 8: the plain
+ * stencil only) - and the site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The other values force one kernel for every
  * call, for parity tests and for timing the variants against each other: ND_STENCIL_SITE; ND_STENCIL_TILE (the tiled kernel
  * above); ND_STENCIL_TILE_TMA (the same kernel with every prefetch issued as a TMA tensor-map box load instead of cp.async; x3
  * extent 32); ND_STENCIL_TILE4 (fp32, x3 extent 32: its predecessor with four link slots and the next spinor in registers).
@@ -286,7 +286,8 @@ ND_API int nd_halo_buffers(nd_ctx* ctx, void** send_next, void** send_prev, void
  *   nd_block_axpy: y <- y + sum_k a[k] v_k           (a = l complex numbers on the host)
  *   nd_gaussian:   fill x with Re, Im ~ N(0,1) from a counter-based generator (Philox-4x32-10 + Box-Muller)
  *   nd_*_dev:      the same reductions with the result left in the caller's DEVICE memory (2l / 2 / 2 doubles, (re, im)
- *                  pairs; nd_norm2_dev: im = 0), enqueued on the context's stream without any synchronisation */
+ *                  pairs; nd_norm2_dev: im = the rounding residue of the cancelling cross terms), and nd_block_axpy with its coefficients read from DEVICE memory (2l doubles):
+ *                  enqueued on the context's stream without any synchronisation, so reductions and updates chain on the device */
 ND_API int nd_axpy(nd_ctx* ctx, const double a[2], const void* x, void* y);
 ND_API int nd_scale(nd_ctx* ctx, const double a[2], void* x);
 ND_API int nd_copy(nd_ctx* ctx, void* y, const void* x);
@@ -298,6 +299,7 @@ ND_API int nd_block_axpy(nd_ctx* ctx, int l, const double* a2l, const void* v, v
 ND_API int nd_block_dot_dev(nd_ctx* ctx, int l, const void* v, const void* x, double* d_out2l);
 ND_API int nd_dot_dev(nd_ctx* ctx, const void* x, const void* y, double* d_out2);
 ND_API int nd_norm2_dev(nd_ctx* ctx, const void* x, double* d_out2);
+ND_API int nd_block_axpy_dev(nd_ctx* ctx, int l, const double* d_a2l, const void* v, void* y);
 ND_API int nd_gaussian(nd_ctx* ctx, void* x, unsigned long long seed);
 
 #ifdef __cplusplus

@@ -82,6 +82,7 @@ SIGNATURES = {
     "nd_block_dot": (_c_int, [_c_vp, _c_int, _c_vp, _c_vp, _pd]),
     "nd_block_axpy": (_c_int, [_c_vp, _c_int, _pd, _c_vp, _c_vp]),
     "nd_block_dot_dev": (_c_int, [_c_vp, _c_int, _c_vp, _c_vp, _c_vp]),
+    "nd_block_axpy_dev": (_c_int, [_c_vp, _c_int, _c_vp, _c_vp, _c_vp]),
     "nd_dot_dev": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp]),
     "nd_norm2_dev": (_c_int, [_c_vp, _c_vp, _c_vp]),
     "nd_gaussian": (_c_int, [_c_vp, _c_vp, _c_ull]),
@@ -532,6 +533,10 @@ class Context:
     def block_dot_dev(self, v, x, out):
         """out: device float64 tensor of 2l entries, (re, im) pairs; no synchronisation."""
         self._chk(self.lib.nd_block_dot_dev(self._h, v.shape[0], v.data_ptr(), x.data_ptr(), out.data_ptr()))
+
+    def block_axpy_dev(self, a, v, y):
+        """a: device float64 tensor of 2l entries, (re, im) pairs; no synchronisation."""
+        self._chk(self.lib.nd_block_axpy_dev(self._h, v.shape[0], a.data_ptr(), v.data_ptr(), y.data_ptr()))
 
     def dot_dev(self, x, y, out):
         self._chk(self.lib.nd_dot_dev(self._h, x.data_ptr(), y.data_ptr(), out.data_ptr()))

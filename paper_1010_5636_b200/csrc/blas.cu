@@ -100,6 +100,8 @@ __global__ void chiral_combine_kernel(typename Prec<T>::Vec* y, const typename P
 //   is read by exactly one thread of the grid), multiplies with the staged columns and accumulates in fp64 registers; one
 //   warp reduction per (k, column) and RANGE, accumulated per CTA in shared memory;
 //   partial[((c*l + k)*2 + {re,im})][cta]  ->  reduce_partials_kernel.  No atomics: bitwise reproducible.
+//   On small lattices with many vectors (16^3x32, l = 50) grid.y splits the block's vectors into chunks so that the machine is
+//   filled through l as well (fp64: 532 -> 287 us).
 struct ColPtrs {
     const void* p[8];
 };
@@ -116,6 +118,9 @@ __global__ void __launch_bounds__(RED_THREADS) block_dot_cols_kernel(double* __r
     double* acc = reinterpret_cast<double*>(dsm + (size_t)NC * NV * DOT_RANGE * sizeof(Vec));   // [nc*l*2] CTA totals
     double* wred = acc + (size_t)2 * NC * l;                                            // [RED_WARPS][2*NC]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // blockIdx.y = chunk of the block's vectors [kb, ke): small lattices with many vectors fill the machine through l as well
+    const int kchunk = (l + (int)gridDim.y - 1) / (int)gridDim.y;
+    const int kb = (int)blockIdx.y * kchunk, ke = (kb + kchunk < l) ? kb + kchunk : l;
     for (int i = threadIdx.x; i < 2 * nc * l; i += blockDim.x) acc[i] = 0.0;
     const long long nranges = (V + DOT_RANGE - 1) / DOT_RANGE;
     for (long long rg = blockIdx.x; rg < nranges; rg += gridDim.x) {
@@ -137,17 +142,27 @@ __global__ void __launch_bounds__(RED_THREADS) block_dot_cols_kernel(double* __r
                 }
         }
         __syncthreads();
-        for (int k = 0; k < l; k++) {
+        for (int k = kb; k < ke; k++) {
             const Vec* vk = v + (long long)k * NV * V;
             double re[NC], im[NC];
 #pragma unroll
             for (int c = 0; c < NC; c++) re[c] = im[c] = 0.0;
+            // fp64: the loads of both sites are issued before the first multiply (853 -> 722 us at 32^3x64, l = 8); fp32: one site
+            // at a time (the same change costs registers there: 325 -> 397 us)
+            cx<T> bb[DOT_SITES_PER_THREAD][12];
+            if (sizeof(T) == 8) {
+#pragma unroll
+                for (int j = 0; j < DOT_SITES_PER_THREAD; j++) {
+                    const long long s = base + j * RED_THREADS + threadIdx.x;
+                    if (s < V) load_site<T>(vk, V, s, bb[j]);
+                }
+            }
 #pragma unroll
             for (int j = 0; j < DOT_SITES_PER_THREAD; j++) {
                 const long long s = base + j * RED_THREADS + threadIdx.x;
                 if (s < V) {
-                    cx<T> b[12];
-                    load_site<T>(vk, V, s, b);
+                    cx<T> (&b)[12] = bb[j];
+                    if (sizeof(T) != 8) load_site<T>(vk, V, s, b);
 #pragma unroll
                     for (int c = 0; c < NC; c++) {
                         if (c < nc) {
@@ -185,7 +200,10 @@ __global__ void __launch_bounds__(RED_THREADS) block_dot_cols_kernel(double* __r
         }
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < 2 * nc * l; i += blockDim.x) partial[(long long)i * gridDim.x + blockIdx.x] = acc[i];
+    for (int i = threadIdx.x; i < 2 * nc * l; i += blockDim.x) {
+        const int k = (i >> 1) % l;
+        if (k >= kb && k < ke) partial[(long long)i * gridDim.x + blockIdx.x] = acc[i];
+    }
 }
 
 // out[i] = sum_b partial[i][b]; one block per i
@@ -427,9 +445,13 @@ int block_dot_cols_t(nd_ctx* ctx, int l, const void* v, int nc, const void* cons
         long long cap = (long long)ND_RESULT_DOUBLES * ND_MAX_RED_BLOCKS / ((long long)2 * l * n);
         if (cap > 8LL * ctx->num_sms) cap = 8LL * ctx->num_sms;
         const unsigned blocks = (unsigned)(nranges < cap ? nranges : cap);
-        if (n == 1) block_dot_cols_kernel<T, 1><<<blocks, RED_THREADS, smem_for(1, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
-        else if (n == 2) block_dot_cols_kernel<T, 2><<<blocks, RED_THREADS, smem_for(2, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
-        else block_dot_cols_kernel<T, NCMAX><<<blocks, RED_THREADS, smem_for(NCMAX, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
+        // few ranges (small lattice) and many vectors: split the vectors over grid.y until there are ~4 CTAs per SM
+        int nkc = 1;
+        while ((long long)blocks * nkc < 4LL * ctx->num_sms && (l + nkc) / (nkc + 1) >= 2) nkc++;
+        const dim3 grid(blocks, (unsigned)nkc, 1);
+        if (n == 1) block_dot_cols_kernel<T, 1><<<grid, RED_THREADS, smem_for(1, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
+        else if (n == 2) block_dot_cols_kernel<T, 2><<<grid, RED_THREADS, smem_for(2, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
+        else block_dot_cols_kernel<T, NCMAX><<<grid, RED_THREADS, smem_for(NCMAX, l), ctx->stream>>>(ctx->d_partial, l, n, (const Vec*)v, cp, ctx->V);
         ND_LAUNCHED(ctx);
         reduce_partials_kernel<<<n * l * 2, RED_THREADS, 0, ctx->stream>>>(d_out + (size_t)2 * l * c0, ctx->d_partial, (int)blocks);
         ND_LAUNCHED(ctx);
@@ -618,6 +640,11 @@ extern "C" int nd_block_axpy(nd_ctx* ctx, int l, const double* a2l, const void* 
     for (int i = 0; i < 2 * l; i++) ctx->h_result[i] = a2l[i];
     ND_CUDA(ctx, cudaMemcpyAsync(ctx->d_coef, ctx->h_result, (size_t)2 * l * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     return ndi_block_axpy_dev(ctx, l, ctx->d_coef, v, y, 0, nullptr, 0.0, 0.0);
+}
+extern "C" int nd_block_axpy_dev(nd_ctx* ctx, int l, const double* d_a2l, const void* v, void* y) {
+    ND_ENTER(ctx);
+    if (l < 1 || l > ND_MAX_BLOCK_L || !d_a2l || !v || !y) return nd_fail(ctx, ND_ERR_BAD_ARG, "block_axpy_dev: bad argument (1 <= l <= %d)", ND_MAX_BLOCK_L);
+    return ndi_block_axpy_dev(ctx, l, d_a2l, v, y, 0, nullptr, 0.0, 0.0);
 }
 extern "C" int nd_gaussian(nd_ctx* ctx, void* x, unsigned long long seed) {
     ND_ENTER(ctx);

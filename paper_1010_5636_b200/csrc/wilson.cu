@@ -324,8 +324,8 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
     }
     // the tiled marching kernel (wilson_tile.cu) where it is the faster one on 32^3x64 (us per launch, tile vs site):
     //   fp32 recon 12 / 8 / 18: plain 139 / 148 / 171 vs 167 / 185 / 196, fused epilogue 224 / 226 / 252 vs 247 / 239 / 279
-    //   fp64 recon 12 / 8: plain 289 / 382 vs 344 / 417; fused 491 / 539 vs 502 / 535 (both at 87-89 % of the HBM peak): plain only
-    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->prec == 32 || !epi))
+    //   fp64 recon 12 / 8: plain 289 / 382 vs 344 / 417; fused 491 / 539 vs 502 / 535 (all at 87-89 % of the HBM peak): fused with recon 12 only
+    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->prec == 32 || !epi || ctx->recon == 12))
                                                                 : (ctx->stencil_variant != ND_STENCIL_SITE);
     if (tile) {   // large lattices: one launch per right-hand side already fills the machine
         const size_t sb = nd_spinor_bytes(ctx);

@@ -89,3 +89,35 @@ def test_gaussian_moments_and_determinism():
     ctx.gaussian(y, 12)
     b = ctx.unpack_spinor(y)
     assert abs(np.vdot(a.ravel(), b.ravel())) < 6 * np.sqrt(n)
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+def test_dev_variants_chain_on_the_device(prec):
+    """nd_block_dot_dev / nd_dot_dev / nd_norm2_dev / nd_block_axpy_dev (results left in device memory): one
+    Gram-Schmidt step x <- x - V (V^dagger x) without any host round trip, against numpy; and the same numbers as the host variants."""
+    import torch
+
+    dims, l = (10, 6, 6, 6), 7
+    ctx, _ = make_context(dims, prec, 12, -1, "smooth")
+    vs = [round_to(gaussian_spinor(dims, seed=40 + k), prec) for k in range(l)]
+    xa = round_to(gaussian_spinor(dims, seed=3), prec)
+    V = ctx.new_spinor(l)
+    for k in range(l):
+        ctx.pack_spinor(vs[k], out=V[k])
+    x = ctx.pack_spinor(xa)
+    with torch.cuda.stream(ctx.stream):
+        c = torch.zeros(2 * l, dtype=torch.float64, device=ctx.torch_device)
+        d2 = torch.zeros(2, dtype=torch.float64, device=ctx.torch_device)
+        n2 = torch.zeros(2, dtype=torch.float64, device=ctx.torch_device)
+        ctx.block_dot_dev(V, x, c)
+        ctx.dot_dev(V[0], x, d2)
+        ctx.norm2_dev(x, n2)
+        host_c = ctx.block_dot(V, x)                  # host variant: synchronises, same kernel
+        cd = c.cpu().numpy()
+        assert np.array_equal(cd[0::2] + 1j * cd[1::2], host_c)
+        assert complex(*d2.cpu().numpy()) == host_c[0] and abs(n2.cpu().numpy()[1]) <= 1e-13 * n2.cpu().numpy()[0]
+        assert abs(n2.cpu().numpy()[0] - np.vdot(xa.ravel(), xa.ravel()).real) <= 1e-12 * n2.cpu().numpy()[0]
+        c.neg_()                                      # on the device, on the context's stream
+        ctx.block_axpy_dev(c, V, x)
+    want = xa - sum(np.vdot(v.ravel(), xa.ravel()) * v for v in vs)
+    assert rel_l2(ctx.unpack_spinor(x), want) <= (1e-13 if prec == 64 else 3e-7)

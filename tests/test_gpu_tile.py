@@ -69,8 +69,8 @@ def test_fp64_tiled_kernel_matches_the_oracle(dims, bc, recon):
         ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])
         fused[variant] = ctx.unpack_spinor(out)
         assert rel_l2(fused[variant], ref_epi) <= TOL[64], variant
-    # auto in fp64: the tiled kernel for the plain stencil, the site-per-thread kernel for the fused-epilogue one
-    assert np.array_equal(results["auto"], results["tile"]) and np.array_equal(fused["auto"], fused["site"])
+    # auto in fp64: the tiled kernel for the plain stencil; for the fused-epilogue one with recon 12 only (site-per-thread with recon 8)
+    assert np.array_equal(results["auto"], results["tile"]) and np.array_equal(fused["auto"], fused["tile" if recon == 12 else "site"])
     assert np.array_equal(results["tile_tma"], results["tile"]) and np.array_equal(fused["tile_tma"], fused["tile"])
     scale = np.abs(ref).max()
     assert np.abs(results["tile"] - ref).max() <= (1e-13 if recon != 8 else 1e-10) * scale
