@@ -164,13 +164,14 @@ struct Solver {
     char* x(int j) { return X + (size_t)j * sb; }
     char* y(int j) { return Y + (size_t)j * sb; }
 
-    int Q(void* out, const void* in) {
-        stencils++;
-        return ndi_apply_Q(ctx, out, in, m, false, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+    // Q and the fused-epilogue Q on n columns stored back to back, one launch for all of them (small lattices: the columns fill the machine)
+    int Qb(int n, void* out, const void* in) {
+        stencils += n;
+        return ndi_apply_Q_batch(ctx, n, out, in, m, false, 1, 0, nullptr, 0, nullptr, 0, nullptr);
     }
-    int Qepi(void* out, const void* in, double a0, double a1, const void* v1, double a2, const void* v2) {
-        stencils++;
-        return ndi_apply_Q(ctx, out, in, m, true, a0, a1, v1, a2, v2, 0, nullptr);
+    int Qepib(int n, void* out, const void* in, double a0, double a1, const void* v1, double a2, const void* v2) {
+        stencils += n;
+        return ndi_apply_Q_batch(ctx, n, out, in, m, true, a0, a1, v1, a2, v2, 0, nullptr);
     }
     // G[i][j] = <A_i, B_j>, i < na, j < nb  -> h_mat row-major (na x nb complex)
     int gram(char* A, int na, char* B, int nb) {
@@ -243,25 +244,26 @@ struct Solver {
     int filter(int d, double low, double lo, double hi, int first) {
         const double c = 0.5 * (hi + lo), e = 0.5 * (hi - lo);
         const double sigma1 = e / (low - c);
-        for (int j = first; j < k; j++) {
-            char* P = x(j);   // t_{i-1}
-            char* R = s0;     // t_i
-            int rc = Q(s1, P);
+        const int n = k - first;              // the same polynomial for every column: all of them in each launch
+        if (n <= 0) return ND_OK;
+        char* P = x(first);                   // t_{i-1}
+        char* R = Z + (size_t)first * sb;     // t_i     (Z and Y are free between two Rayleigh-Ritz steps)
+        char* tmp = y(first);
+        int rc = Qb(n, tmp, P);
+        if (rc != ND_OK) return rc;
+        rc = Qepib(n, R, tmp, sigma1 / e, -c * sigma1 / e, P, 0.0, nullptr);   // t_1
+        if (rc != ND_OK) return rc;
+        double sigma = sigma1;
+        for (int i = 1; i < d; i++) {
+            const double sn = 1.0 / (2.0 / sigma1 - sigma);
+            rc = Qb(n, tmp, R);
             if (rc != ND_OK) return rc;
-            rc = Qepi(R, s1, sigma1 / e, -c * sigma1 / e, P, 0.0, nullptr);   // t_1
+            rc = Qepib(n, P, tmp, 2.0 * sn / e, -2.0 * sn * c / e, R, -sigma * sn, P);   // t_{i+1} over t_{i-1}
             if (rc != ND_OK) return rc;
-            double sigma = sigma1;
-            for (int i = 1; i < d; i++) {
-                const double sn = 1.0 / (2.0 / sigma1 - sigma);
-                rc = Q(s1, R);
-                if (rc != ND_OK) return rc;
-                rc = Qepi(P, s1, 2.0 * sn / e, -2.0 * sn * c / e, R, -sigma * sn, P);   // t_{i+1} over t_{i-1}
-                if (rc != ND_OK) return rc;
-                std::swap(P, R);
-                sigma = sn;
-            }
-            // d even: t_d sits in x(j) again
+            std::swap(P, R);
+            sigma = sn;
         }
+        // d even: t_d sits in X again
         return ND_OK;
     }
 };
@@ -321,7 +323,7 @@ extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l_min, int l_max, int lguard
             if (rc != ND_OK) return finish(rc);
         }
         // Y = Q X;  H = Y^dagger Y = X^dagger Q^2 X: its extreme eigenvalues are the extreme Ritz values of Q^2 in the block
-        for (int j = 0; j < k && rc == ND_OK; j++) rc = S.Q(S.y(j), S.x(j));
+        rc = S.Qb(k, S.Y, S.X);
         if (rc == ND_OK) rc = S.gram(S.Y, k, S.Y, k);
         if (rc != ND_OK) return finish(rc);
         Hm.assign(S.h_mat.begin(), S.h_mat.end());
@@ -355,7 +357,7 @@ extern "C" int nd_lowmodes_compute(nd_ctx* ctx, int l_min, int l_max, int lguard
         if (rc != ND_OK) return finish(rc);
         std::swap(S.X, S.Z);
         // residues rho_j = ||(Q - nu_j) u_j|| of the whole block (eq. 2.8), Q u_j recomputed on the rotated vectors
-        for (int j = 0; j < k && rc == ND_OK; j++) rc = S.Q(S.y(j), S.x(j));
+        rc = S.Qb(k, S.Y, S.X);
         if (rc == ND_OK) rc = ndi_block_resid(ctx, k, S.X, S.Y, nu, rho.data());
         if (rc != ND_OK) return finish(rc);
         for (int j = 0; j < k; j++) {
