@@ -170,8 +170,10 @@ __device__ __forceinline__ void cx_to_words(const cx<double> (&c)[12], double2 (
 // ---------------------------------------------------------------------------- internal entry points (per TU)
 int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
                 double s2, const void* v2, double s3, const void* v3);
-bool ndi_tile_supported(const nd_ctx* ctx);
-int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
+bool ndi_tile_supported(const nd_ctx* ctx);                 // geometry and, for one right-hand side, enough sites
+bool ndi_tile_geometry(const nd_ctx* ctx);
+bool ndi_tile_worthwhile(const nd_ctx* ctx, int nrhs);
+int ndi_apply_Q_tile(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                      const void* v2, double s3, const void* v3);
 int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
                       double s2, const void* v2, double s3, const void* v3);

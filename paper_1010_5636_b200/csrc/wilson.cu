@@ -325,18 +325,12 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
     // the tiled marching kernel (wilson_tile.cu) where it is the faster one on 32^3x64 (us per launch, tile vs site):
     //   fp32 recon 12 / 8 / 18: plain 139 / 148 / 171 vs 167 / 185 / 196, fused epilogue 224 / 226 / 252 vs 247 / 239 / 279
     //   fp64 recon 12 / 8: plain 289 / 382 vs 344 / 417; fused 491 / 539 vs 502 / 535 (all at 87-89 % of the HBM peak): fused with recon 12 only
-    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO) ? (ctx->tile_ok && (ctx->prec == 32 || !epi || ctx->recon == 12))
-                                                                : (ctx->stencil_variant != ND_STENCIL_SITE);
-    if (tile) {   // large lattices: one launch per right-hand side already fills the machine
-        const size_t sb = nd_spinor_bytes(ctx);
-        for (int j = 0; j < nrhs; j++) {
-            const size_t o = (size_t)j * sb;
-            int rc = ndi_apply_Q_tile(ctx, (char*)out + o, (const char*)in + o, m, epi, s0, s1, v1 ? (const char*)v1 + o : nullptr, s2,
-                                      v2 ? (const char*)v2 + o : nullptr, s3, v3 ? (const char*)v3 + o : nullptr);
-            if (rc != ND_OK) return rc;
-        }
-        return ND_OK;
-    }
+    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO)
+                          ? (ndi_tile_geometry(ctx) && ndi_tile_worthwhile(ctx, nrhs) && (ctx->prec == 32 || !epi || ctx->recon == 12))
+                          : (ctx->stencil_variant != ND_STENCIL_SITE);
+    // (a batch of right-hand sides on a small lattice marches as many columns as one source on a large one: 16^3x32 takes the
+    // tiled kernel from 2 sources on)
+    if (tile) return ndi_apply_Q_tile(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
 #define ND_DISPATCH(T, R) return launch_Q<T, R>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3, nrhs)
     if (ctx->prec == 32) {
         if (ctx->recon == 18) ND_DISPATCH(float, 18);

@@ -510,10 +510,15 @@ __global__ void __launch_bounds__(128, MINB)
     wilson_Q_tile2_kernel(typename Prec<T>::Vec* out, const typename Prec<T>::Vec* __restrict__ in,
                           const typename LinkLayout<T, RECON>::LVec* __restrict__ gauge, TileGeom G, T mass_term, T s0, T s1,
                           const typename Prec<T>::Vec* v1, T s2, const typename Prec<T>::Vec* v2, T s3,
-                          const typename Prec<T>::Vec* v3) {
+                          const typename Prec<T>::Vec* v3, long long batch_stride) {
     using Vec = typename Prec<T>::Vec;
     using LL = LinkLayout<T, RECON>;
     using LVec = typename LL::LVec;
+    {   // blockIdx.y = right-hand side of a batch stored back to back (the links are shared through L2)
+        const long long off = (long long)blockIdx.y * batch_stride;
+        out += off; in += off;
+        if (EPI) { if (v1) v1 += off; if (v2) v2 += off; if (v3) v3 += off; }
+    }
     // x3 extent 32: one 2 x 2 x 32 tile per CTA, a warp is one x3 row; x3 extent 16: two independent 2 x 2 x 16 tiles per CTA
     // (neighbours in x2), a warp is the two rows (r2 = 0, 1) of one r1: the x2 partner of a site is in its own warp
     constexpr int NT = 128, NSUB = 32 / L3, SUBT = NT / NSUB;
@@ -684,7 +689,7 @@ __global__ void __launch_bounds__(128, MINB)
 }
 
 template <typename T, int RECON, bool EPI, int MINB, int L3>
-int launch_tile2(nd_ctx* ctx, void* out, const void* in, double m, double s0, double s1, const void* v1, double s2, const void* v2,
+int launch_tile2(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, double s0, double s1, const void* v1, double s2, const void* v2,
                  double s3, const void* v3) {
     using Vec = typename Prec<T>::Vec;
     using LL = LinkLayout<T, RECON>;
@@ -709,12 +714,13 @@ int launch_tile2(nd_ctx* ctx, void* out, const void* in, double m, double s0, do
         if (n < 1) return nd_fail(ctx, ND_ERR_CUDA, "tiled fp64 stencil does not fit on an SM");
         per_sm = n;
     }
-    const int nseg = choose_segments(G.L0, G.ntile, per_sm * ctx->num_sms);
+    const int nseg = choose_segments(G.L0, G.ntile * nrhs, per_sm * ctx->num_sms);   // a batch = more columns to march along
     G.seg_base = G.L0 / nseg;
     G.seg_rem = G.L0 % nseg;
-    const unsigned blocks = (unsigned)(G.ntile * nseg);
+    const dim3 blocks((unsigned)(G.ntile * nseg), (unsigned)nrhs, 1);
     kern<<<blocks, NT, smem, ctx->stream>>>((Vec*)out, (const Vec*)in, (const LVec*)ctx->gauge, G, T(4.0 + m), T(s0), T(s1),
-                                            (const Vec*)v1, T(s2), (const Vec*)v2, T(s3), (const Vec*)v3);
+                                            (const Vec*)v1, T(s2), (const Vec*)v2, T(s3), (const Vec*)v3,
+                                            (long long)Prec<T>::NV * ctx->V);
     ND_LAUNCHED(ctx);
     return ND_OK;
 }
@@ -1099,26 +1105,29 @@ int launch_tile_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi
 // (at least ND_TILE_MIN_CTA_SLICES_PER_SM slices of 128 sites per SM: below that the segments along x0 get so short that their
 // prologue - one extra spinor and link per column - eats the gain; 16^3x32 has 6.9 and runs 12.3 us site vs 14.4 us tiled in fp32)
 constexpr long long ND_TILE_MIN_CTA_SLICES_PER_SM = 8;
-bool ndi_tile_supported(const nd_ctx* ctx) {
+bool ndi_tile_geometry(const nd_ctx* ctx) {
     const int L1 = ctx->dims[1], L2 = ctx->dims[2], L3 = ctx->dims[3];
     if (L3 != 32 && L3 != 16) return false;
     if (L1 % 2 != 0 || L2 % (64 / L3) != 0) return false;      // x3 extent 16: a CTA takes two tiles side by side in x2
     if (L1 < 4 || L2 < 4) return false;
     if (ctx->prec == 64 && ctx->recon == 18) return false;
-    return ctx->V / 128 >= ND_TILE_MIN_CTA_SLICES_PER_SM * ctx->num_sms;
+    return true;
 }
+// ... for nrhs right-hand sides per launch (a batch on a small lattice is as good as one source on a large one)
+bool ndi_tile_worthwhile(const nd_ctx* ctx, int nrhs) { return ctx->V * nrhs / 128 >= ND_TILE_MIN_CTA_SLICES_PER_SM * ctx->num_sms; }
+bool ndi_tile_supported(const nd_ctx* ctx) { return ndi_tile_geometry(ctx) && ndi_tile_worthwhile(ctx, 1); }
 
 // fp32: 3 CTAs of 128 threads per SM for the plain stencil (145 registers), 2 for the fused epilogue (the three update vectors of
 // the site are loaded before the last barrier); fp64: 2 CTAs per SM (255 registers, 105 KB shared memory)
 template <typename T, int RECON, int MINB, int MINB_EPI>
-static int launch_tile2_shape(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
-                              const void* v2, double s3, const void* v3) {
+static int launch_tile2_shape(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
+                              double s2, const void* v2, double s3, const void* v3) {
     if (ctx->dims[3] == 16) {
-        if (epi) return launch_tile2<T, RECON, true, MINB_EPI, 16>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
-        return launch_tile2<T, RECON, false, MINB, 16>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+        if (epi) return launch_tile2<T, RECON, true, MINB_EPI, 16>(ctx, nrhs, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile2<T, RECON, false, MINB, 16>(ctx, nrhs, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
     }
-    if (epi) return launch_tile2<T, RECON, true, MINB_EPI, 32>(ctx, out, in, m, s0, s1, v1, s2, v2, s3, v3);
-    return launch_tile2<T, RECON, false, MINB, 32>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+    if (epi) return launch_tile2<T, RECON, true, MINB_EPI, 32>(ctx, nrhs, out, in, m, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile2<T, RECON, false, MINB, 32>(ctx, nrhs, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
 }
 
 template <typename T, int RECON, int MINB, int MINB_EPI>
@@ -1130,8 +1139,19 @@ static int launch_tile3_shape(nd_ctx* ctx, void* out, const void* in, double m, 
 
 // ND_STENCIL_TILE (and auto): the two-slot kernel wilson_Q_tile2_kernel; ND_STENCIL_TILE_TMA: the same schedule with tensor-map
 // loads, wilson_Q_tile3_kernel (x3 extent 32); ND_STENCIL_TILE4 (fp32, x3 extent 32): the four-slot kernel wilson_Q_tile_kernel
-int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
+int ndi_apply_Q_tile(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                      const void* v2, double s3, const void* v3) {
+    if (nrhs > 1 && (ctx->stencil_variant == ND_STENCIL_TILE_TMA || ctx->stencil_variant == ND_STENCIL_TILE4)) {
+        // the variants kept for comparison take one right-hand side per launch
+        const size_t sb = nd_spinor_bytes(ctx);
+        for (int j = 0; j < nrhs; j++) {
+            const size_t o = (size_t)j * sb;
+            const int rc = ndi_apply_Q_tile(ctx, 1, (char*)out + o, (const char*)in + o, m, epi, s0, s1, v1 ? (const char*)v1 + o : nullptr, s2,
+                                            v2 ? (const char*)v2 + o : nullptr, s3, v3 ? (const char*)v3 + o : nullptr);
+            if (rc != ND_OK) return rc;
+        }
+        return ND_OK;
+    }
     if (ctx->stencil_variant == ND_STENCIL_TILE_TMA) {
         if (ctx->prec == 64) {
             if (ctx->recon == 12) return launch_tile3_shape<double, 12, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
@@ -1142,15 +1162,15 @@ int ndi_apply_Q_tile(nd_ctx* ctx, void* out, const void* in, double m, bool epi,
         return launch_tile3_shape<float, 8, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
     }
     if (ctx->prec == 64) {
-        if (ctx->recon == 12) return launch_tile2_shape<double, 12, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
-        return launch_tile2_shape<double, 8, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        if (ctx->recon == 12) return launch_tile2_shape<double, 12, 2, 2>(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+        return launch_tile2_shape<double, 8, 2, 2>(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
     }
     if (ctx->stencil_variant == ND_STENCIL_TILE4) {
         if (ctx->recon == 18) return launch_tile_shape<18>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
         if (ctx->recon == 12) return launch_tile_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
         return launch_tile_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
     }
-    if (ctx->recon == 18) return launch_tile2_shape<float, 18, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
-    if (ctx->recon == 12) return launch_tile2_shape<float, 12, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
-    return launch_tile2_shape<float, 8, 3, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    if (ctx->recon == 18) return launch_tile2_shape<float, 18, 3, 2>(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    if (ctx->recon == 12) return launch_tile2_shape<float, 12, 3, 2>(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    return launch_tile2_shape<float, 8, 3, 2>(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
 }
