@@ -693,6 +693,16 @@ def run_b200(args):
         cpu = cpu_baseline_sample(dims=dims, U=U64)
         ncores = os.cpu_count() or 1
         cpu["q_alone"] = [oracle_q_alone_subprocess(lat, th) for lat in ("16^3x32", "32^3x64") for th in (1, ncores)]
+        # the oracle's D_N on the lattices of BASELINE configs 3 and 4 (SURVEY.md 8(d) "CPU baseline"): the full degree of config 3,
+        # a bounded degree and fewer vectors for config 4 (its full n = 200, l = 50 would take minutes in numpy)
+        from lattice_inputs import gauge_field as _gf
+
+        cpu["dn_configs"] = []
+        for idx, cd, feps, cn, cl in ((3, (16, 8, 8, 8), 0.3, 100, 8), (4, (32, 16, 16, 16), 0.25, 40, 4)):
+            r = cpu_baseline_sample(n=cn, l=cl, dims=cd, U=_gf(cd, "smooth", eps=feps))
+            cpu["dn_configs"].append({"config_index": idx, "lattice": f"{cd[1]}^3x{cd[0]}", "degree": cn, "vectors": cl, "cores": r["cores"],
+                                      "seconds_per_dn": r["seconds_per_step"], "gflops_1320": r["value"],
+                                      "tau_ns_per_clenshaw_iteration_per_site": r["tau_ns_per_clenshaw_iteration_per_site"]})
     elif not args.no_cpu_baseline:
         cpu = cpu_baseline_sample(dims=(32, 16, 16, 16), n=6)
     line = {
