@@ -687,7 +687,7 @@ def run_b200(args):
         projection = [measure_projection(torch, nd, "32^3x64", 8, 32, peak), measure_projection(torch, nd, "16^3x32", 50, 32, peak),
                       measure_projection(torch, nd, "16^3x32", 50, 64, peak)]
         configs.append(q_config(torch, nd))
-        configs.append(dn_config(torch, nd, 3, "8^3x16", 64, 0.3, (16, 24), 8, 100, 60, 1e-6, nrhs=8))
+        configs.append(dn_config(torch, nd, 3, "8^3x16", 64, 0.3, (16, 24), 8, 100, 60, 1e-6, nrhs=10))
         configs.append(dn_config(torch, nd, 4, "16^3x32", 32, 0.25, (44, 56), 12, 200, 160, 1e-2, nrhs=4))
     if not args.no_cpu_baseline and not args.quick:
         cpu = cpu_baseline_sample(dims=dims, U=U64)
