@@ -19,7 +19,13 @@
 //     them while the current slice is computed: a whole slice of link data per CTA is in flight without holding registers;
 //   * x1 and x2 use separate exchange buffers in turn (send x1, barrier, receive x1, send x2, barrier, receive x2): two
 //     __syncthreads per time-slice and no buffer is ever written while it may still be read.
-// L2 -> SM traffic per site (fp32, recon 12, tile 2 x 4 x 32): 288 own + 96 store + 180 halo = 564 B; tile 4 x 4 x 32: 504 B.
+// L2 -> SM traffic per site (fp32, recon 12, tile 2 x 2 x 32, measured): 541 B against 822 B of the site-per-thread kernel.
+//
+// Three kernels share this scheme:
+//   wilson_Q_tile_kernel   the first shipped form (fp32): four link slots, next spinor of the column in registers (ND_STENCIL_TILE4)
+//   wilson_Q_tile2_kernel  the default (fp32 and fp64, x3 extent 32 or 16, batches of right-hand sides): two link slots shared by
+//                          two directions each, next spinor through a shared-memory slot, four cp.async groups per slice
+//   wilson_Q_tile3_kernel  tile2's schedule with TMA tensor-map box loads instead of cp.async (ND_STENCIL_TILE_TMA)
 #include <cuda.h>   // CUtensorMap (the tensor-map variant at the end of this file)
 
 #include "nd_dirac.cuh"
