@@ -17,6 +17,7 @@ roofline = the dominant kernel (the Q stencil), timed alone with CUDA events on 
            (median of 5 batches, clocks sampled meanwhile), against the measured HBM copy peak of MEASURED_PEAKS.json;
            `q_kernel` holds every precision x recon variant and, for fp32, the stencil variants against each other.
 layout   = a1 alone: pack / unpack / link compression, GB/s over AoS + SoA bytes.
+next_rows = SURVEY 8(f): D_N^m inversion (fp64 CG, mixed precision), index by zero-mode counting, min-max coefficients.
 projection = a7 alone: block dot and block axpy over l vectors (32^3x64 l = 8; 16^3x32 l = 50), GB/s over the compulsory bytes.
 configs  = the other timed BASELINE.json configurations, driver-run in the same line: index 1 (1000 back-to-back Q on
            16^3x32, fp32 + fp64 x recon 12 / 8), index 3 (D_N on 8^3x16, fp64, about 20 modes from the library's
@@ -343,6 +344,67 @@ def measure_projection(torch, nd, lattice, l, prec, peak):
         res[k]["frac_of_measured_peak"] = res[k]["gbs"] / peak
     ctx.close()
     del Vb, x, c, a
+    torch.cuda.empty_cache()
+    return res
+
+
+def measure_next_rows(torch, nd):
+    """The SURVEY.md 8(f) rows beyond D_N itself, timed through the C ABI (parity of each is in tests/): f2 inversion of the massive
+    operator D_N^m by CG on the normal equations in fp64 and with fp32 inner / fp64 outer refinement, f2 index by zero-mode
+    counting on a constant-flux field, f4 min-max against interpolation coefficients (host utilities)."""
+    from lattice_inputs import flux_su3, gauge_field
+
+    res = {}
+    # ---- f2: inversion on 8^3x16 (BASELINE config 3's lattice), no projected modes, quark mass 0.1
+    dims, n, eps, mq = (16, 8, 8, 8), 100, 0.0045, 0.1
+    U = gauge_field(dims, "smooth", eps=0.3)
+    c, delta = nd.cheb_coeffs(n, eps)
+    c64 = nd.Context(dims, prec=64, recon=12, bc_time=-1)
+    c32 = nd.Context(dims, prec=32, recon=12, bc_time=-1)
+    c64.set_gauge(U)
+    c32.set_gauge(U.astype(np.complex64))
+    for cc in (c64, c32):
+        cc.set_sign_poly(c, eps, QNORM, M_KERNEL)
+        cc.set_lowmodes(None, [])
+    b, x = c64.new_spinor(), c64.new_spinor()
+    c64.gaussian(b, 5636)
+    c64.synchronize()
+    t0 = time.perf_counter()
+    relres, iters, ok = c64.solve_DNm(x, b, RHO, mq, tol=1e-8, maxit=400)
+    c64.synchronize()
+    t1 = time.perf_counter()
+    relres_m, outer, inner, ok_m = c64.solve_DNm_mixed(c32, x, b, RHO, mq, tol=1e-8, inner_tol=1e-3)
+    c64.synchronize()
+    t2 = time.perf_counter()
+    res["f2_inversion"] = {"lattice": "8^3x16", "degree": n, "eps": eps, "delta": delta, "quark_mass": mq, "tol": 1e-8,
+                           "fp64_cg": {"seconds": t1 - t0, "iterations": iters, "relres": relres, "converged": ok,
+                                       "sign_applications": 2 * iters + 2},
+                           "mixed": {"seconds": t2 - t1, "outer_steps": outer, "fp32_cg_iterations": inner, "relres": relres_m,
+                                     "converged": ok_m}}
+    c64.close()
+    c32.close()
+    # ---- f2: index on a constant-flux field (|index| = 2 |q01 q23| = 2), low modes and sign function from the library
+    dims = (8, 8, 4, 4)
+    ctx = nd.Context(dims, prec=64, recon=12, bc_time=-1)
+    ctx.set_gauge(flux_su3(dims, 1, 1, noise=0.05))
+    ctx.synchronize()
+    t0 = time.perf_counter()
+    u, nu, resid, st = ctx.lowmodes_compute(2, M_KERNEL, tol=1e-8, maxit=80, lextra=6, degree=20, l_max=8, stop="residue")
+    guard = float(np.abs(st["nu_guard"]).min())
+    eps = 0.99 * guard ** 2 / QNORM ** 2
+    c, delta = nd.cheb_coeffs(80, eps)
+    ctx.set_sign_poly(c, eps, QNORM, M_KERNEL)
+    ctx.set_lowmodes(u, nu)
+    npl, nmi, ist = ctx.index_count(6, 1e-3, degree=8, maxit=40)
+    ctx.synchronize()
+    res["f2_index"] = {"lattice": "8x8x4x4 constant-flux field (q01 = q23 = 1, 5 % noise)", "n_plus": npl, "n_minus": nmi, "index": npl - nmi,
+                       "seconds": time.perf_counter() - t0, "projected_modes": int(st["l_chosen"]), "sign_applications": ist["sign_applications"],
+                       "lowest_nonzero": float(min(e for e in ist["evals"].ravel() if e > 1e-3))}
+    ctx.close()
+    # ---- f4: min-max (Remez) against interpolation coefficients at the headline's degree
+    ci, di = nd.cheb_coeffs(100, 0.002)
+    cm, dm, lev = nd.minmax_coeffs(100, 0.002)
+    res["f4_minmax"] = {"degree": 100, "eps": 0.002, "delta_interpolation": di, "delta_minmax": dm, "levelled_error": lev}
     torch.cuda.empty_cache()
     return res
 
@@ -689,7 +751,7 @@ def run_b200(args):
                 "timing": "median of 5 batches of 20 launches, CUDA events on the launch stream; first leg of the run (before the D_N legs)",
                 "frac_of_8TBs_nominal": main["achieved_gbs"] / 8000.0, "clocks": q_clocks,
                 "traffic_source": "profiles/q_kernel_dram_traffic.csv (ncu --set full of this kernel on this lattice; null = no capture)"}
-    layout, projection, configs, cpu = None, None, [], None
+    layout, projection, configs, cpu, next_rows = None, None, [], None, None
     if not args.quick:
         layout = {f"f{p}": measure_layout(torch, nd, dims, U64, p, peak) for p in (32, 64)}
         projection = [measure_projection(torch, nd, "32^3x64", 8, 32, peak), measure_projection(torch, nd, "16^3x32", 50, 32, peak),
@@ -697,6 +759,7 @@ def run_b200(args):
         configs.append(q_config(torch, nd))
         configs.append(dn_config(torch, nd, 3, "8^3x16", 64, 0.3, (16, 24), 8, 100, 60, 1e-6, nrhs=10))
         configs.append(dn_config(torch, nd, 4, "16^3x32", 32, 0.25, (44, 56), 12, 200, 160, 1e-2, nrhs=4))
+        next_rows = measure_next_rows(torch, nd)
     if not args.no_cpu_baseline and not args.quick:
         cpu = cpu_baseline_sample(dims=dims, U=U64)
         ncores = os.cpu_count() or 1
@@ -741,6 +804,7 @@ def run_b200(args):
         "q_kernel": qk,
         "layout": layout,
         "projection": projection,
+        "next_rows": next_rows,
         "configs": configs,
         "cpu_baseline": cpu,
     }
