@@ -159,6 +159,24 @@ __global__ void __launch_bounds__(256) wilson_Q_hop_kernel(typename Prec<T>::Vec
     const int lane = threadIdx.x, hop = threadIdx.y;
     const long long s = (long long)blockIdx.x * 32 + lane;
     const bool valid = s < G.V;
+    // the planes this warp will finish (hop, hop + 8): the site's own spinor and the fused update's vectors are requested NOW,
+    // so that their latency runs concurrently with the hop's own load -> multiply chain instead of after the barrier
+    constexpr int NPW = (NV + 7) / 8;
+    Vec phi_p[NPW], vp[3][NPW];
+    if (valid) {
+#pragma unroll
+        for (int k = 0; k < NPW; k++) {
+            const int p = hop + 8 * k;
+            if (p < NV) {
+                phi_p[k] = in[p * G.V + s];
+                if (EPI) {
+                    if (v1) vp[0][k] = v1[p * G.V + s];
+                    if (v2) vp[1][k] = v2[p * G.V + s];
+                    if (v3) vp[2][k] = v3[p * G.V + s];
+                }
+            }
+        }
+    }
     cx<T> acc[12];
 #pragma unroll
     for (int i = 0; i < 12; i++) acc[i] = {T(0), T(0)};
@@ -192,30 +210,33 @@ __global__ void __launch_bounds__(256) wilson_Q_hop_kernel(typename Prec<T>::Vec
     }
     __syncthreads();
     if (!valid) return;
-    for (int p = hop; p < NV; p += 8) {   // warp `hop` finishes planes hop, hop + 8
-        Vec phi = in[p * G.V + s], w;
+#pragma unroll
+    for (int k = 0; k < NPW; k++) {   // warp `hop` finishes planes hop, hop + 8
+        const int p = hop + 8 * k;
+        if (p >= NV) break;
+        Vec phi = phi_p[k], w;
         const T* pr = reinterpret_cast<const T*>(&phi);
         T* wr = reinterpret_cast<T*>(&w);
         const T sg = (p * W < 12) ? T(1) : T(-1);   // gamma5: reals 0..11 are spin 0, 1
 #pragma unroll
-        for (int k = 0; k < W; k++) {
+        for (int q = 0; q < W; q++) {
             T t = T(0);
 #pragma unroll
-            for (int h = 0; h < 8; h++) t += red[h][p * W + k][lane];
-            wr[k] = sg * fma(T(-0.5), t, mass_term * pr[k]);
+            for (int h = 0; h < 8; h++) t += red[h][p * W + q][lane];
+            wr[q] = sg * fma(T(-0.5), t, mass_term * pr[q]);
         }
         if (EPI) {
 #pragma unroll
-            for (int k = 0; k < W; k++) wr[k] *= s0;
+            for (int q = 0; q < W; q++) wr[q] *= s0;
             const Vec* vs[3] = {v1, v2, v3};
             const T ss[3] = {s1, s2, s3};
 #pragma unroll
             for (int j = 0; j < 3; j++)
                 if (vs[j]) {
-                    Vec a = vs[j][p * G.V + s];
+                    const Vec a = vp[j][k];
                     const T* ar = reinterpret_cast<const T*>(&a);
 #pragma unroll
-                    for (int k = 0; k < W; k++) wr[k] = fma(ss[j], ar[k], wr[k]);
+                    for (int q = 0; q < W; q++) wr[q] = fma(ss[j], ar[q], wr[q]);
                 }
         }
         out[p * G.V + s] = w;
