@@ -77,6 +77,30 @@ def test_set_gauge_rejects_non_su3():
     assert e.value.code == -2
 
 
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("where", ["one entry", "a whole warp of links"])
+def test_set_gauge_rejects_nan_links(prec, where):
+    """A NaN anywhere in the links must fail the SU(3) check (fmax / fmin drop NaN operands and `x > tol` is false for NaN: the
+    device statistics map NaN to +inf and the host test is written as !(x <= tol)); nd_gauge_stats reports +inf."""
+    import paper_1010_5636_b200 as nd
+
+    dims = (4, 4, 4, 8)
+    U = gauge_field(dims, "haar")
+    if where == "one entry":
+        U[1, 2, 3, 0, 5, 1, 2] = np.nan
+    else:
+        U[3, 0, 0, 0:2] = np.nan            # 64 consecutive links of one direction: every lane of two warps
+    ctx = nd.Context(dims, prec=prec, recon=12)
+    with pytest.raises(nd.NDError) as e:
+        ctx.set_gauge(U if prec == 64 else U.astype(np.complex64))
+    assert e.value.code == -3
+    st = ctx.gauge_stats()
+    assert np.isinf(st[0]) and np.isinf(st[1])
+    with pytest.raises(nd.NDError) as e:
+        ctx.apply_Q(ctx.new_spinor(), ctx.new_spinor(), 0.1)
+    assert e.value.code == -2
+
+
 @pytest.mark.parametrize("dims", [(6, 4, 2, 10), (4, 6, 12, 2), (2, 2, 2, 2), (10, 6, 6, 6)])
 @pytest.mark.parametrize("recon", [12, 8])
 @pytest.mark.parametrize("prec", [64, 32])
