@@ -1123,7 +1123,7 @@ bool ndi_tile_geometry(const nd_ctx* ctx) {
 bool ndi_tile_worthwhile(const nd_ctx* ctx, int nrhs) { return ctx->V * nrhs / 128 >= ND_TILE_MIN_CTA_SLICES_PER_SM * ctx->num_sms; }
 bool ndi_tile_supported(const nd_ctx* ctx) { return ndi_tile_geometry(ctx) && ndi_tile_worthwhile(ctx, 1); }
 
-// fp32: 3 CTAs of 128 threads per SM for the plain stencil (145 registers), 2 for the fused epilogue (the three update vectors of
+// fp32: 3 CTAs of 128 threads per SM for the plain stencil (145 - 161 registers), 2 for the fused epilogue (the three update vectors of
 // the site are loaded before the last barrier); fp64: 2 CTAs per SM (255 registers, 105 KB shared memory)
 template <typename T, int RECON, int MINB, int MINB_EPI>
 static int launch_tile2_shape(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,
