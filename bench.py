@@ -258,6 +258,8 @@ def measure_q_kernel(torch, nd, dims, lattice, U64, prec, recon, peak, variants=
         ms, batches = median_of_batches(torch, ctx, lambda: ctx.apply_Q(y, x, M_KERNEL), reps)
         gbs = q_bytes_per_site(prec, recon) * V / (ms * 1e-3) / 1e9
         kernel = stencil_kernel_name(name, V, prec)
+        if var is None and name == "tile" and prec == 64 and recon == 8 and dims[3] == 32:
+            kernel = "wilson_Q_tile3_kernel"   # auto: tensor-map loads for the plain fp64 recon-8 stencil
         r = {"prec": prec, "recon": recon, "stencil_variant": name, "kernel": kernel, "us_per_launch": ms * 1e3,
              "us_per_launch_batches": [b * 1e3 for b in batches], "gflops_1320": FLOP_PER_SITE * V / (ms * 1e-3) / 1e9,
              "bytes_per_site": q_bytes_per_site(prec, recon), "achieved_gbs": gbs, "frac_of_measured_peak": gbs / peak,

@@ -74,7 +74,7 @@ ND_API size_t nd_gauge_bytes(const nd_ctx* ctx);        /* bytes of the compress
  * picks the fastest one measured for the context and call: the tiled marching kernel (neighbour exchange through shared memory,
  * cp.async prefetch of links, halos and the next spinor) on lattices it supports - x3 extent 32 or 16, even x1 / x2 extents >= 4
  * (x3 extent 16: x2 extent divisible by 4), at least 8 slices of 128 sites per SM, in fp64 recon 12 / 8 (recon 8: the plain
- * stencil only) - and the site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The other values force one kernel for every
+ * stencil only, with tensor-map loads on x3 extent 32) - and the site-per-thread kernel otherwise (hop-parallel below 16384 sites).  The other values force one kernel for every
  * call, for parity tests and for timing the variants against each other: ND_STENCIL_SITE; ND_STENCIL_TILE (the tiled kernel
  * above); ND_STENCIL_TILE_TMA (the same kernel with every prefetch issued as a TMA tensor-map box load instead of cp.async; x3
  * extent 32); ND_STENCIL_TILE4 (fp32, x3 extent 32: its predecessor with four link slots and the next spinor in registers).

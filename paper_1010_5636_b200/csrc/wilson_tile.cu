@@ -1158,7 +1158,10 @@ int ndi_apply_Q_tile(nd_ctx* ctx, int nrhs, void* out, const void* in, double m,
         }
         return ND_OK;
     }
-    if (ctx->stencil_variant == ND_STENCIL_TILE_TMA) {
+    // (auto: the tensor-map loads are the faster ones for the plain fp64 stencil with recon 8 - 363 vs 382 us on 32^3x64 - where
+    // the per-thread cp.async address arithmetic competes with the 8-parameter reconstruction for issue slots)
+    const bool auto_tma = ctx->stencil_variant == ND_STENCIL_AUTO && ctx->prec == 64 && ctx->recon == 8 && !epi && nrhs == 1 && ctx->dims[3] == 32;
+    if (ctx->stencil_variant == ND_STENCIL_TILE_TMA || auto_tma) {
         if (ctx->prec == 64) {
             if (ctx->recon == 12) return launch_tile3_shape<double, 12, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
             return launch_tile3_shape<double, 8, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
