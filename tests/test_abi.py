@@ -183,3 +183,40 @@ def test_minmax_coeffs_match_oracle(n, eps):
     else:
         ci, di = nd.cheb_coeffs(n, eps)
         assert delta < 0.75 * di
+
+
+def test_header_is_plain_c_and_links_from_c(tmp_path):
+    """The boundary is a C ABI: include/nd_b200.h compiles as strict C99 (no C++-isms, no torch types), a plain-C program links
+    against libnd_b200.so, and without a CUDA device nd_create fails with ND_ERR_CUDA and a NULL context instead of crashing
+    (there is no CPU fallback).  On a GPU box the same program creates and destroys a context."""
+    import shutil
+    import subprocess
+
+    import paper_1010_5636_b200 as nd
+
+    if shutil.which("gcc") is None:
+        pytest.skip("no gcc")
+    nd.load_library()
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    src = tmp_path / "abi_smoke.c"
+    src.write_text(
+        '#include <stdio.h>\n#include "nd_b200.h"\n'
+        "int main(void) {\n"
+        "    nd_ctx* ctx = (nd_ctx*)0;\n"
+        "    const int dims[4] = {4, 4, 4, 4};\n"
+        "    double c[9], delta = 0.0;\n"
+        "    int rc = nd_cheb_coeffs(8, 0.1, c, &delta);          /* host utility: works without a GPU */\n"
+        "    if (rc != ND_OK || !(delta > 0.0 && delta < 1.0)) return 3;\n"
+        "    rc = nd_create(&ctx, dims, 64, 12, -1, 0, (void*)0);\n"
+        '    printf("%d %d %lld\\n", rc, ctx != (nd_ctx*)0, rc == ND_OK ? nd_volume(ctx) : -1LL);\n'
+        "    if (rc == ND_OK) return nd_destroy(ctx) == ND_OK ? 0 : 4;\n"
+        "    return (rc == ND_ERR_CUDA && ctx == (nd_ctx*)0) ? 0 : 5;\n"
+        "}\n")
+    exe = tmp_path / "abi_smoke"
+    libdir = os.path.dirname(nd.LIB_PATH)
+    subprocess.run(["gcc", "-std=c99", "-pedantic", "-Wall", "-Wextra", "-Werror", "-I", os.path.join(root, "include"), str(src), "-o", str(exe),
+                    "-L", libdir, "-lnd_b200", "-Wl,-rpath," + libdir], check=True, capture_output=True, text=True)
+    r = subprocess.run([str(exe)], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0, (r.returncode, r.stdout, r.stderr)
+    rc, have_ctx, vol = (int(x) for x in r.stdout.split())
+    assert (rc, have_ctx, vol) in ((0, 1, 256), (-5, 0, -1))
