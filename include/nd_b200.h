@@ -7,7 +7,8 @@
  * Conventions
  * -----------
  *  - Opaque context; EVERY call returns an int status (ND_OK = 0, negative = error).  No exceptions, no
- *    global state.  nd_last_error(ctx) gives a human-readable message owned by the context.
+ *    global state (one exception, stated there: the static scratch array of nd_dot_static).  nd_last_error(ctx) gives a
+ *    human-readable message owned by the context.
  *  - Field memory is CALLER-OWNED DEVICE memory (e.g. torch tensors' data_ptr()).  A device spinor occupies
  *    nd_spinor_bytes(ctx) bytes and must be 16-byte aligned.  The context owns only: the compressed gauge
  *    field, reduction scratch, polynomial coefficients, a *pointer* to the caller's low-mode block.
@@ -301,6 +302,33 @@ ND_API int nd_dot_dev(nd_ctx* ctx, const void* x, const void* y, double* d_out2)
 ND_API int nd_norm2_dev(nd_ctx* ctx, const void* x, double* d_out2);
 ND_API int nd_block_axpy_dev(nd_ctx* ctx, int l, const double* d_a2l, const void* v, void* y);
 ND_API int nd_gaussian(nd_ctx* ctx, void* x, unsigned long long seed);
+
+/* ------------------------------------------------------------- inner product without any memory allocation
+ * nd_dot_static: d_out2 = <x, y> = sum conj(x) y over two device SoA spinors of V sites (the BLAS-1 reduction of the
+ * Clenshaw / low-mode steps), for callers that must not allocate device memory: a plug-in inside an
+ * application whose own pool already holds the GPU's memory, code in a phase where cudaMalloc / cudaFree (which synchronise
+ * the device) are off limits, a process with a fixed memory budget.  Every other reduction needs a context, and nd_create
+ * calls cudaMalloc; this call needs no context and calls no cudaMalloc, cudaFree or any other allocating routine, ever.
+ * Its partial sums go to an array that is part of the library image: ND_DOT_STATIC_SCRATCH_BYTES of device memory on every
+ * GPU that loads the library's kernels, held until the process exits.
+ *   x, y     [in, device]  SoA spinors of `prec` (32: 6 planes of float4[V], 64: 12 planes of double2[V]), 16-byte aligned
+ *   V        sites, 1 <= V <= ND_DOT_STATIC_MAX_SITES (one partial sum per 256 sites must fit the array; 32^3 x 128 fits);
+ *            anything else is refused with ND_ERR_BAD_ARG and a message naming the limit
+ *   prec     32 or 64; products and sums are formed in fp64 in both cases
+ *   device   CUDA device ordinal the pointers belong to (the caller's current device is restored before returning)
+ *   stream   cudaStream_t as void* (may be NULL); the two kernels are enqueued there, nothing is synchronised
+ *   d_out2   [out, device] 2 doubles (re, im), caller-owned, written by the second kernel
+ *   errbuf   [out, host, may be NULL] receives a message of at most errbuf_len bytes when the call fails ("" on success)
+ * Returns ND_OK, ND_ERR_BAD_ARG or ND_ERR_CUDA.  The result is bitwise reproducible and agrees with nd_dot_dev to rounding
+ * (a different, equally fixed summation order).  On a sharded lattice it is the LOCAL sum - there is no context to reduce over.
+ * The first call on each device looks up the array's device address (cudaGetSymbolAddress, cached afterwards): make that
+ * first call outside any stream capture.  All calls on a device share the one array: a call overwrites the slots it later
+ * reads, so nothing needs clearing between calls, but two calls that can overlap on the GPU (two streams, two host threads)
+ * race on it - keep them on one stream or order them yourself. */
+#define ND_DOT_STATIC_MAX_SITES 4194304
+#define ND_DOT_STATIC_SCRATCH_BYTES 262144
+ND_API int nd_dot_static(const void* x, const void* y, long long V, int prec, int device, void* stream, double* d_out2,
+                         char* errbuf, size_t errbuf_len);
 
 #ifdef __cplusplus
 }

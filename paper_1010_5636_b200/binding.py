@@ -86,7 +86,11 @@ SIGNATURES = {
     "nd_dot_dev": (_c_int, [_c_vp, _c_vp, _c_vp, _c_vp]),
     "nd_norm2_dev": (_c_int, [_c_vp, _c_vp, _c_vp]),
     "nd_gaussian": (_c_int, [_c_vp, _c_vp, _c_ull]),
+    "nd_dot_static": (_c_int, [_c_vp, _c_vp, _c_ll, _c_int, _c_int, _c_vp, _c_vp, ctypes.c_char_p, _c_sz]),
 }
+
+DOT_STATIC_MAX_SITES = 4194304          # ND_DOT_STATIC_MAX_SITES
+DOT_STATIC_SCRATCH_BYTES = 262144       # ND_DOT_STATIC_SCRATCH_BYTES
 
 EXCHANGE_START_FN = ctypes.CFUNCTYPE(_c_int, _c_vp, _c_vp, _c_vp, _c_vp, _c_vp, _c_sz)
 EXCHANGE_WAIT_FN = ctypes.CFUNCTYPE(_c_int, _c_vp)
@@ -203,6 +207,20 @@ def _ptr(x):
     if isinstance(x, int):
         return x
     return x.data_ptr()      # torch tensor
+
+
+def dot_static(x, y, V, prec, out, device=0, stream=None):
+    """nd_dot_static: out[0:2] = <x, y> (re, im) for two device SoA spinors of V sites, without a context and without
+    any allocation - for callers that may not call cudaMalloc (memory owned by someone else's pool, allocator calls
+    forbidden in the current phase, fixed memory budget).  The partial sums use a 256 KiB array inside the library image,
+    shared by all calls on the device: keep calls that could overlap on one stream.  V <= DOT_STATIC_MAX_SITES.
+    x, y, out: device tensors or raw device addresses; stream: a torch stream, a raw cudaStream_t or None."""
+    lib = load_library()
+    st = getattr(stream, "cuda_stream", stream)
+    err = ctypes.create_string_buffer(512)
+    rc = lib.nd_dot_static(_ptr(x), _ptr(y), int(V), int(prec), int(device), _c_vp(st), _ptr(out), err, len(err))
+    if rc != ND_OK:
+        raise NDError(rc, err.value.decode())
 
 
 def _c2(a):

@@ -14,7 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnd_b200.so")
-SOURCES = ["api.cu", "layout.cu", "wilson.cu", "wilson_tile.cu", "shard.cu", "blas.cu", "sign.cu", "lowmodes.cu", "solver.cu"]
+SOURCES = ["api.cu", "layout.cu", "wilson.cu", "wilson_tile.cu", "shard.cu", "blas.cu", "sign.cu", "lowmodes.cu", "solver.cu",
+           "dot_static.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # IEEE arithmetic: no --use_fast_math anywhere
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
