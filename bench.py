@@ -257,9 +257,8 @@ def measure_q_kernel(torch, nd, dims, lattice, U64, prec, recon, peak, variants=
         name = ctx.get_stencil_variant()
         ms, batches = median_of_batches(torch, ctx, lambda: ctx.apply_Q(y, x, M_KERNEL), reps)
         gbs = q_bytes_per_site(prec, recon) * V / (ms * 1e-3) / 1e9
+        name = ctx.get_stencil_variant_for(False, 1)     # the dispatch's own choice for this call (auto depends on the call)
         kernel = stencil_kernel_name(name, V, prec)
-        if var is None and name == "tile" and prec == 64 and recon == 8 and dims[3] == 32:
-            kernel = "wilson_Q_tile3_kernel"   # auto: tensor-map loads for the plain fp64 recon-8 stencil
         r = {"prec": prec, "recon": recon, "stencil_variant": name, "kernel": kernel, "us_per_launch": ms * 1e3,
              "us_per_launch_batches": [b * 1e3 for b in batches], "gflops_1320": FLOP_PER_SITE * V / (ms * 1e-3) / 1e9,
              "bytes_per_site": q_bytes_per_site(prec, recon), "achieved_gbs": gbs, "frac_of_measured_peak": gbs / peak,
@@ -274,7 +273,7 @@ def measure_q_kernel(torch, nd, dims, lattice, U64, prec, recon, peak, variants=
                 ctx.gaussian(v[j], 77 + j)
             msf, _ = median_of_batches(torch, ctx, lambda: ctx.apply_Q_axpbycz(v[1], x, M_KERNEL, 0.05, -0.9, v[0], -0.5, v[1], 0.01, v[2]), reps)
             gbf = q_bytes_per_site(prec, recon, 3) * V / (msf * 1e-3) / 1e9
-            out["fused_epilogue"] = {"kernel": stencil_kernel_name("site" if (prec == 64 and recon != 12 and var is None) else name, V, prec),
+            out["fused_epilogue"] = {"kernel": stencil_kernel_name(ctx.get_stencil_variant_for(True, 1), V, prec),
                                      "us_per_launch": msf * 1e3, "bytes_per_site": q_bytes_per_site(prec, recon, 3),
                                      "achieved_gbs": gbf, "frac_of_measured_peak": gbf / peak, "frac_of_8TBs": gbf / 8000.0}
             del v
@@ -452,7 +451,7 @@ def dn_config(torch, nd, index, lattice, prec, field_eps, l_window, guard, n, ei
          "sources": sources, "dn_applies_per_s": sources / (ms * 1e-3), "ms_per_dn": ms / sources,
          "gflops_1320": FLOP_PER_SITE * V * (2 * n + 1) * sources / (ms * 1e-3) / 1e9,
          "tau_ns_per_clenshaw_iteration_per_site": ms * 1e6 / sources / (n * V),
-         "kernel": stencil_kernel_name(ctx.get_stencil_variant(), V, prec)}
+         "kernel": stencil_kernel_name(ctx.get_stencil_variant_for(True, 1), V, prec)}
     if nrhs > 1:
         nb = min(nrhs, sources)
         workb = ctx.new_spinor(3 * nb)
@@ -487,7 +486,7 @@ def q_config(torch, nd, lattice="16^3x32", field_eps=0.3, reps=1000):
         runs[f"f{prec}_recon{recon}"] = {"ms_for_1000": ms, "us_per_Q": ms * 1e3 / reps,
                                          "gflops_1320": FLOP_PER_SITE * V * reps / (ms * 1e-3) / 1e9,
                                          "model_gbs": q_bytes_per_site(prec, recon) * V * reps / (ms * 1e-3) / 1e9,
-                                         "kernel": stencil_kernel_name(ctx.get_stencil_variant(), V, prec)}
+                                         "kernel": stencil_kernel_name(ctx.get_stencil_variant_for(False, 1), V, prec)}
         ctx.close()
         del x, y
     torch.cuda.empty_cache()

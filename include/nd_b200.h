@@ -80,10 +80,14 @@ ND_API size_t nd_gauge_bytes(const nd_ctx* ctx);        /* bytes of the compress
  * above); ND_STENCIL_TILE_TMA (the same kernel with every prefetch issued as a TMA tensor-map box load instead of cp.async; x3
  * extent 32); ND_STENCIL_TILE4 (fp32, x3 extent 32: its predecessor with four link slots and the next spinor in registers).
  * ND_ERR_BAD_ARG if the context cannot run it.  Cached CUDA graphs are dropped.  nd_get_stencil_variant returns the variant in
- * effect for the plain stencil (never ND_STENCIL_AUTO). */
+ * effect for the plain stencil on lattices the tiled kernels take (never ND_STENCIL_AUTO); under ND_STENCIL_AUTO the choice also
+ * depends on the call, and nd_get_stencil_variant_for answers for one call exactly - nd_apply_Q (fused_epilogue = 0) or
+ * nd_apply_Q_axpbycz / the Clenshaw steps (fused_epilogue != 0) on nrhs right-hand sides - through the very function the dispatch
+ * uses: ND_STENCIL_SITE covers the site-per-thread and, below 16384 sites x nrhs, the hop-parallel kernel. */
 enum { ND_STENCIL_AUTO = 0, ND_STENCIL_SITE = 1, ND_STENCIL_TILE = 2, ND_STENCIL_TILE_TMA = 3, ND_STENCIL_TILE4 = 4 };
 ND_API int nd_set_stencil_variant(nd_ctx* ctx, int variant);
 ND_API int nd_get_stencil_variant(const nd_ctx* ctx);
+ND_API int nd_get_stencil_variant_for(const nd_ctx* ctx, int fused_epilogue, int nrhs);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 ND_API long long nd_launch_count(const nd_ctx* ctx);
 

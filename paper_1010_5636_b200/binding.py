@@ -43,6 +43,7 @@ SIGNATURES = {
     "nd_halo_buffers": (_c_int, [_c_vp, ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp), ctypes.POINTER(_c_vp)]),
     "nd_set_stencil_variant": (_c_int, [_c_vp, _c_int]),
     "nd_get_stencil_variant": (_c_int, [_c_vp]),
+    "nd_get_stencil_variant_for": (_c_int, [_c_vp, _c_int, _c_int]),
     "nd_set_gauge": (_c_int, [_c_vp, _c_vp, _c_int, _c_int]),
     "nd_get_gauge": (_c_int, [_c_vp, _c_vp, _c_int]),
     "nd_gauge_stats": (_c_int, [_c_vp, _pd]),
@@ -343,6 +344,13 @@ class Context:
 
     def get_stencil_variant(self):
         v = int(self.lib.nd_get_stencil_variant(self._h))
+        return {n: k for k, n in self.STENCIL.items()}[v]
+
+    def get_stencil_variant_for(self, fused_epilogue=False, nrhs=1):
+        """The variant one call runs (plain / fused-epilogue stencil on nrhs right-hand sides): the dispatch's own choice."""
+        v = int(self.lib.nd_get_stencil_variant_for(self._h, int(bool(fused_epilogue)), int(nrhs)))
+        if v < 0:
+            raise NDError(v, "nd_get_stencil_variant_for")
         return {n: k for k, n in self.STENCIL.items()}[v]
 
     def launch_count(self):

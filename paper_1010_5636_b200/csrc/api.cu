@@ -76,6 +76,8 @@ extern "C" int nd_create(nd_ctx** out, const int dims[4], int prec, int recon, i
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device);
     ctx->err[0] = 0;
     for (int i = 0; i < 8; i++) ctx->tile_ctas_per_sm[i] = 0;
+    for (int i = 0; i < ND_TMAP_SLOTS; i++) ctx->tmaps[i].base = nullptr;
+    ctx->tmap_next = 0;
     ctx->tile_ok = ndi_tile_supported(ctx);
     ctx->stencil_variant = ND_STENCIL_AUTO;
     ctx->dot_configured = false;
@@ -157,6 +159,11 @@ extern "C" int nd_get_stencil_variant(const nd_ctx* ctx) {
     if (!ctx) return ND_ERR_BAD_ARG;
     if (ctx->stencil_variant != ND_STENCIL_AUTO) return ctx->stencil_variant;
     return ctx->tile_ok ? ND_STENCIL_TILE : ND_STENCIL_SITE;
+}
+
+extern "C" int nd_get_stencil_variant_for(const nd_ctx* ctx, int fused_epilogue, int nrhs) {
+    if (!ctx || nrhs < 1) return ND_ERR_BAD_ARG;
+    return ndi_select_stencil(ctx, fused_epilogue != 0, nrhs);
 }
 
 extern "C" long long nd_volume(const nd_ctx* ctx) { return ctx ? ctx->V : 0; }

@@ -28,6 +28,15 @@ struct nd_graph_entry {
     int nrhs;
 };
 
+// A cached CUtensorMap of the tensor-map stencil (wilson_tile.cu): the map encodes only the base address and the shape of the
+// array, so it stays valid for as long as an array of that shape lives at that address (nd_set_gauge rewrites the links in place).
+struct nd_tmap_slot {
+    const void* base;       // nullptr: empty
+    int word_bytes, planes, box_planes;
+    alignas(64) unsigned char map[128];   // CUtensorMap, kept opaque here (cuda.h is included by wilson_tile.cu only)
+};
+constexpr int ND_TMAP_SLOTS = 8;
+
 struct nd_ctx {
     int dims[4];
     long long V;
@@ -63,6 +72,8 @@ struct nd_ctx {
     bool dot_configured;        // block_dot_cols_kernel shared-memory attributes set
     bool tile_ok;               // the tiled marching stencil (wilson_tile.cu) takes this lattice
     int stencil_variant;        // ND_STENCIL_* (nd_set_stencil_variant)
+    nd_tmap_slot tmaps[ND_TMAP_SLOTS];   // link map + the spinor maps of the last few `in` pointers, replaced round robin
+    int tmap_next;
     int tile_ctas_per_sm[8];    // resident CTAs per SM of the tiled kernels ({four-slot, -, two-slot, tensor map} x {plain, fused}), 0 = not queried yet
     // domain decomposition along x0 (shard.cu): this context is the local lattice of rank shard_rank of shard_n
     int shard_rank, shard_n;
@@ -173,6 +184,9 @@ int ndi_apply_Q(nd_ctx* ctx, void* out, const void* in, double m, bool epi, doub
 bool ndi_tile_supported(const nd_ctx* ctx);                 // geometry and, for one right-hand side, enough sites
 bool ndi_tile_geometry(const nd_ctx* ctx);
 bool ndi_tile_worthwhile(const nd_ctx* ctx, int nrhs);
+// THE choice of stencil kernel for one call (plain / fused epilogue, nrhs right-hand sides): ND_STENCIL_SITE, _TILE, _TILE_TMA or
+// _TILE4, never _AUTO.  The dispatch in wilson.cu / wilson_tile.cu and nd_get_stencil_variant_for both go through it.
+int ndi_select_stencil(const nd_ctx* ctx, bool epi, int nrhs);
 int ndi_apply_Q_tile(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                      const void* v2, double s3, const void* v3);
 int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1,

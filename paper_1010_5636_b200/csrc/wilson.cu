@@ -335,23 +335,22 @@ int ndi_apply_Q_batch(nd_ctx* ctx, int nrhs, void* out, const void* in, double m
                                    v2 ? (const char*)v2 + o : nullptr, s3, v3 ? (const char*)v3 + o : nullptr);
             ctx->bc = saved_bc;
             ctx->in_shard_call = false;
-            if (rc != ND_OK) return rc;
-            if (ctx->exchange_wait(ctx->comm_user) != 0) return nd_fail(ctx, ND_ERR_CUDA, "sharding: the exchange-wait callback failed");
-            rc = ndi_halo_apply(ctx, (char*)out + o, epi ? s0 : 1.0);
-            if (rc != ND_OK) return rc;
+            // From here on the exchange is under way on every rank (requests posted / faces stored into the neighbours' windows):
+            // whatever happened to the local stencil, complete it and move to the other half of the receive windows, so that
+            // no request is left outstanding, no peer waits for ever and halo_parity stays the same on all ranks.  The first
+            // error is the one reported.
+            if (!ctx->exchange_wait || ctx->exchange_wait(ctx->comm_user) != 0) {
+                if (rc == ND_OK) rc = nd_fail(ctx, ND_ERR_CUDA, "sharding: the exchange-wait callback failed");
+            } else if (rc == ND_OK) {
+                rc = ndi_halo_apply(ctx, (char*)out + o, epi ? s0 : 1.0);
+            }
             ctx->halo_parity ^= 1;   // the next application uses the other half of the receive windows
+            if (rc != ND_OK) return rc;
         }
         return ND_OK;
     }
-    // the tiled marching kernel (wilson_tile.cu) where it is the faster one on 32^3x64 (us per launch, tile vs site):
-    //   fp32 recon 12 / 8 / 18: plain 139 / 148 / 171 vs 167 / 185 / 196, fused epilogue 224 / 226 / 252 vs 247 / 239 / 279
-    //   fp64 recon 12 / 8: plain 289 / 382 vs 344 / 417; fused 491 / 539 vs 502 / 535 (all at 87-89 % of the HBM peak): fused with recon 12 only
-    const bool tile = (ctx->stencil_variant == ND_STENCIL_AUTO)
-                          ? (ndi_tile_geometry(ctx) && ndi_tile_worthwhile(ctx, nrhs) && (ctx->prec == 32 || !epi || ctx->recon == 12))
-                          : (ctx->stencil_variant != ND_STENCIL_SITE);
-    // (a batch of right-hand sides on a small lattice marches as many columns as one source on a large one: 16^3x32 takes the
-    // tiled kernel from 2 sources on)
-    if (tile) return ndi_apply_Q_tile(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
+    // tiled marching kernels (wilson_tile.cu) or the site-per-thread / hop-parallel kernels of this file: ndi_select_stencil
+    if (ndi_select_stencil(ctx, epi, nrhs) != ND_STENCIL_SITE) return ndi_apply_Q_tile(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
 #define ND_DISPATCH(T, R) return launch_Q<T, R>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3, nrhs)
     if (ctx->prec == 32) {
         if (ctx->recon == 18) ND_DISPATCH(float, 18);

@@ -28,6 +28,9 @@
 //   wilson_Q_tile3_kernel  tile2's schedule with TMA tensor-map box loads instead of cp.async (ND_STENCIL_TILE_TMA)
 #include <cuda.h>   // CUtensorMap (the tensor-map variant at the end of this file)
 
+#include <cstring>
+#include <mutex>
+
 #include "nd_dirac.cuh"
 
 namespace {
@@ -994,15 +997,31 @@ __global__ void __launch_bounds__(128, MINB)
 typedef CUresult (*nd_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                        const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                        CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-int make_row_map(nd_ctx* ctx, CUtensorMap* tm, const void* base, int word_bytes, int planes, int box_planes) {
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda), resolved once per process
+nd_encode_tiled_fn tensor_map_encoder() {
+    static std::once_flag once;
     static nd_encode_tiled_fn encode = nullptr;
-    if (!encode) {
+    std::call_once(once, [] {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult q;
-        ND_CUDA(ctx, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
-        if (!fn || q != cudaDriverEntryPointSuccess) return nd_fail(ctx, ND_ERR_CUDA, "cuTensorMapEncodeTiled is not available in this driver");
-        encode = (nd_encode_tiled_fn)fn;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess && fn && q == cudaDriverEntryPointSuccess)
+            encode = (nd_encode_tiled_fn)fn;
+    });
+    return encode;
+}
+// The maps are cached in the context (nd_tmap_slot): the link map is encoded once, spinor maps once per `in` pointer among the
+// last ND_TMAP_SLOTS arrays - the Clenshaw loop cycles through four - so a launch outside a CUDA graph makes no driver call.
+int make_row_map(nd_ctx* ctx, CUtensorMap* tm, const void* base, int word_bytes, int planes, int box_planes) {
+    static_assert(sizeof(CUtensorMap) == sizeof(nd_tmap_slot::map), "opaque copy of CUtensorMap in nd_internal.cuh");
+    for (int i = 0; i < ND_TMAP_SLOTS; i++) {
+        const nd_tmap_slot& c = ctx->tmaps[i];
+        if (c.base == base && c.word_bytes == word_bytes && c.planes == planes && c.box_planes == box_planes) {
+            memcpy(tm, c.map, sizeof(CUtensorMap));
+            return ND_OK;
+        }
     }
+    const nd_encode_tiled_fn encode = tensor_map_encoder();
+    if (!encode) return nd_fail(ctx, ND_ERR_CUDA, "cuTensorMapEncodeTiled is not available in this driver");
     const int rb = ctx->prec / 8;                                   // bytes of a real
     const cuuint64_t row = (cuuint64_t)ctx->dims[3] * word_bytes;   // bytes of an x3 row of one plane
     const cuuint64_t dims[5] = {row / rb, (cuuint64_t)ctx->dims[2], (cuuint64_t)ctx->dims[1], (cuuint64_t)ctx->dims[0], (cuuint64_t)planes};
@@ -1013,6 +1032,10 @@ int make_row_map(nd_ctx* ctx, CUtensorMap* tm, const void* base, int word_bytes,
                               dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                               CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return nd_fail(ctx, ND_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    nd_tmap_slot& c = ctx->tmaps[ctx->tmap_next];
+    ctx->tmap_next = (ctx->tmap_next + 1) % ND_TMAP_SLOTS;
+    c.base = base; c.word_bytes = word_bytes; c.planes = planes; c.box_planes = box_planes;
+    memcpy(c.map, tm, sizeof(CUtensorMap));
     return ND_OK;
 }
 
@@ -1143,7 +1166,22 @@ static int launch_tile3_shape(nd_ctx* ctx, void* out, const void* in, double m, 
     return launch_tile3<T, RECON, false, MINB>(ctx, out, in, m, 1, 0, nullptr, 0, nullptr, 0, nullptr);
 }
 
-// ND_STENCIL_TILE (and auto): the two-slot kernel wilson_Q_tile2_kernel; ND_STENCIL_TILE_TMA: the same schedule with tensor-map
+// Which kernel one stencil call runs.  Auto = the fastest measured on 32^3x64 (us per launch, tile vs site):
+//   fp32 recon 12 / 8 / 18: plain 139 / 148 / 171 vs 167 / 185 / 196, fused epilogue 224 / 226 / 252 vs 247 / 239 / 279
+//   fp64 recon 12 / 8: plain 289 / 382 vs 344 / 417; fused 491 / 539 vs 502 / 535 (all at 87-89 % of the HBM peak): fused with recon 12 only
+//   fp64 recon 8, plain, one source, x3 extent 32: the tensor-map loads (363 vs 382 us) - the per-thread cp.async address arithmetic
+//   competes with the 8-parameter reconstruction for issue slots
+// A batch of right-hand sides on a small lattice marches as many columns as one source on a large one (ndi_tile_worthwhile): 16^3x32
+// takes the tiled kernel from 2 sources on.
+int ndi_select_stencil(const nd_ctx* ctx, bool epi, int nrhs) {
+    const int v = ctx->stencil_variant;
+    if (v != ND_STENCIL_AUTO) return (v == ND_STENCIL_TILE4 && ctx->prec == 64) ? (int)ND_STENCIL_TILE : v;   // (nd_set_stencil_variant refuses that pair)
+    if (!(ndi_tile_geometry(ctx) && ndi_tile_worthwhile(ctx, nrhs) && (ctx->prec == 32 || !epi || ctx->recon == 12))) return ND_STENCIL_SITE;
+    if (ctx->prec == 64 && ctx->recon == 8 && !epi && nrhs == 1 && ctx->dims[3] == 32) return ND_STENCIL_TILE_TMA;
+    return ND_STENCIL_TILE;
+}
+
+// ND_STENCIL_TILE: the two-slot kernel wilson_Q_tile2_kernel; ND_STENCIL_TILE_TMA: the same schedule with tensor-map
 // loads, wilson_Q_tile3_kernel (x3 extent 32); ND_STENCIL_TILE4 (fp32, x3 extent 32): the four-slot kernel wilson_Q_tile_kernel
 int ndi_apply_Q_tile(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, bool epi, double s0, double s1, const void* v1, double s2,
                      const void* v2, double s3, const void* v3) {
@@ -1158,10 +1196,8 @@ int ndi_apply_Q_tile(nd_ctx* ctx, int nrhs, void* out, const void* in, double m,
         }
         return ND_OK;
     }
-    // (auto: the tensor-map loads are the faster ones for the plain fp64 stencil with recon 8 - 363 vs 382 us on 32^3x64 - where
-    // the per-thread cp.async address arithmetic competes with the 8-parameter reconstruction for issue slots)
-    const bool auto_tma = ctx->stencil_variant == ND_STENCIL_AUTO && ctx->prec == 64 && ctx->recon == 8 && !epi && nrhs == 1 && ctx->dims[3] == 32;
-    if (ctx->stencil_variant == ND_STENCIL_TILE_TMA || auto_tma) {
+    const int sel = ndi_select_stencil(ctx, epi, nrhs);
+    if (sel == ND_STENCIL_TILE_TMA) {
         if (ctx->prec == 64) {
             if (ctx->recon == 12) return launch_tile3_shape<double, 12, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
             return launch_tile3_shape<double, 8, 2, 2>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
@@ -1174,7 +1210,7 @@ int ndi_apply_Q_tile(nd_ctx* ctx, int nrhs, void* out, const void* in, double m,
         if (ctx->recon == 12) return launch_tile2_shape<double, 12, 2, 2>(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
         return launch_tile2_shape<double, 8, 2, 2>(ctx, nrhs, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
     }
-    if (ctx->stencil_variant == ND_STENCIL_TILE4) {
+    if (sel == ND_STENCIL_TILE4) {
         if (ctx->recon == 18) return launch_tile_shape<18>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
         if (ctx->recon == 12) return launch_tile_shape<12>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);
         return launch_tile_shape<8>(ctx, out, in, m, epi, s0, s1, v1, s2, v2, s3, v3);

@@ -144,3 +144,25 @@ def test_variant_selection_rules():
     ctx64b, _ = make_context((40, 2, 16, 32), 64, 12)                # fp64 tiles need x1 / x2 extents >= 4
     with pytest.raises(nd.NDError):
         ctx64b.set_stencil_variant("tile")
+
+
+def test_variant_for_one_call_is_the_dispatch_choice():
+    """nd_get_stencil_variant_for answers for ONE call through the function the dispatch itself uses: under auto
+    the kernel depends on precision, link form, plain / fused epilogue and the number of right-hand sides."""
+    dims = (40, 8, 16, 32)
+    c32, _ = make_context(dims, 32, 8)
+    assert [c32.get_stencil_variant_for(e, 1) for e in (False, True)] == ["tile", "tile"]
+    c64_12, _ = make_context(dims, 64, 12)
+    assert [c64_12.get_stencil_variant_for(e, 1) for e in (False, True)] == ["tile", "tile"]
+    c64_8, _ = make_context(dims, 64, 8)
+    assert c64_8.get_stencil_variant_for(False, 1) == "tile_tma"      # plain fp64 recon 8: tensor-map loads
+    assert c64_8.get_stencil_variant_for(False, 2) == "tile"          # ... one source per launch only
+    assert c64_8.get_stencil_variant_for(True, 1) == "site"           # fused fp64 recon 8: the site kernel
+    c64_18, _ = make_context(dims, 64, 18)
+    assert [c64_18.get_stencil_variant_for(e, 1) for e in (False, True)] == ["site", "site"]   # no fp64 recon-18 tile
+    small, _ = make_context((32, 16, 16, 16), 32, 12)                 # 16^3 x 32: tiled from two sources on
+    assert small.get_stencil_variant_for(False, 1) == "site" and small.get_stencil_variant_for(False, 2) == "tile"
+    for forced in ("site", "tile", "tile_tma"):
+        c32.set_stencil_variant(forced)
+        assert [c32.get_stencil_variant_for(e, n) for e in (False, True) for n in (1, 3)] == [forced] * 4
+    assert c32.lib.nd_get_stencil_variant_for(c32._h, 0, 0) == -1
