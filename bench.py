@@ -285,6 +285,36 @@ def measure_q_kernel(torch, nd, dims, lattice, U64, prec, recon, peak, variants=
     return out
 
 
+def sharded_probe(torch, nd, world, rank, local, p2p):
+    """One stencil application on a tiny lattice split over the ranks (the transports bench.py is about to use), compared with
+    the same lattice applied whole on this GPU: every site of the rank's part, and the global norm - which crosses the
+    all-reduce and depends on both received faces - identical on all ranks by construction of the check."""
+    from paper_1010_5636_b200.dist import make_comm
+
+    gd = (4 * world, 4, 4, 8)
+    U = gauge_field(gd, "smooth", eps=0.3)
+    tb, tl, _, _ = nd.shard_layout(gd[0], world, rank)
+    whole = nd.Context(gd, prec=64, recon=12, bc_time=-1, device=local)
+    whole.set_gauge(U)
+    x, y = whole.new_spinor(), whole.new_spinor()
+    whole.gaussian(x, 99)
+    whole.apply_Q(y, x, M_KERNEL)
+    ref_norm, xa, ya = whole.norm2(y), whole.unpack_spinor(x), whole.unpack_spinor(y)
+    part = nd.Context((tl,) + gd[1:], prec=64, recon=12, bc_time=-1, device=local)
+    part.set_gauge(np.ascontiguousarray(U[:, tb:tb + tl]))
+    comm, kind = make_comm(part, p2p=p2p)
+    xl, yl = part.pack_spinor(np.ascontiguousarray(xa[tb:tb + tl])), part.new_spinor()
+    part.apply_Q(yl, xl, M_KERNEL)
+    got_norm = part.norm2(yl)
+    err = float(np.abs(part.unpack_spinor(yl) - ya[tb:tb + tl]).max())
+    part.close()
+    whole.close()
+    del comm
+    if not (abs(got_norm - ref_norm) <= 1e-10 * ref_norm and err <= 1e-12 * np.sqrt(ref_norm)):
+        raise RuntimeError(f"sharded stencil disagrees with the whole lattice: |y|^2 {got_norm} vs {ref_norm}, worst entry {err}")
+    return kind
+
+
 def measure_layout(torch, nd, dims, U64, prec, peak):
     """a1 alone (VERDICT r1 task 6): AoS <-> SoA on the device, link compression; GB/s over the bytes of both sides."""
     ctx = nd.Context(dims, prec=prec, recon=12, bc_time=-1)
@@ -583,9 +613,24 @@ def run_b200(args):
     # BASELINE config index 2: Haar-random links, seeded (--field smooth for the exp(i eps H) recipe)
     U64 = gauge_field(gdims, args.field, eps=args.field_eps)
     decompose = world > 1 and not args.replicas
+    comm_kind, shard_fallback = None, None
+    if decompose:
+        # Before anything is sized for the decomposition: one tiny sharded stencil checked against the same lattice on this GPU
+        # alone, the verdict agreed between the ranks.  If the transports cannot be set up here (or give wrong faces), the run
+        # falls back to N independent replicas and says so, rather than hanging or failing in the headline path.
+        from paper_1010_5636_b200.dist import CommSetupError, run_agreed
+
+        try:
+            run_agreed(lambda: sharded_probe(torch, nd, world, rank, local, args.p2p), "sharded probe",
+                       torch.device("cuda", local))
+        except CommSetupError as e:
+            shard_fallback = str(e)
+            decompose = False
+            if rank == 0:
+                print(f"bench.py: domain decomposition unavailable ({e}); running {world} replicas instead", file=sys.stderr)
     if decompose:
         # domain decomposition: this rank's time-slices of the one global lattice (nd_shard_layout), faces over NCCL
-        from paper_1010_5636_b200.dist import PeerComm, TorchDistComm
+        from paper_1010_5636_b200.dist import make_comm
 
         tb, tl, _, _ = nd.shard_layout(gdims[0], world, rank)
         dims = (tl,) + tuple(gdims[1:])
@@ -609,7 +654,9 @@ def run_b200(args):
     ctx = nd.Context(dims, prec=prec, recon=recon, bc_time=-1, device=local)
     ctx.set_gauge(Uloc.astype(np.complex64) if prec == 32 else Uloc)
     # from here on every call acts on the global lattice; --p2p: faces stored by the pack kernel into the neighbours' windows
-    comm = (PeerComm(ctx) if args.p2p else TorchDistComm(ctx)) if decompose else None
+    comm = None
+    if decompose:
+        comm, comm_kind = make_comm(ctx, p2p=args.p2p)    # (p2p falls back to NCCL send/recv with the reason on stderr)
     V = ctx.V                                             # sites of this rank
     c, delta = nd.cheb_coeffs(n, args.eps)
     ctx.set_sign_poly(c, args.eps, QNORM, M_KERNEL)
@@ -786,8 +833,8 @@ def run_b200(args):
                    "lattice": args.lattice, "sites": V_global, "sites_per_gpu": V, "recon": recon, "degree": n, "eps": args.eps,
                    "delta": delta, "lowmodes": l, "lowmodes_kind": modes_kind, "stencil_variant": headline_variant,
                    "parallelism": (f"domain decomposition along x0 over {world} GPUs ({gdims[0] // world} slices each), "
-                                   f"half-spinor faces {'stored peer-to-peer into symmetric memory' if args.p2p else 'over NCCL'}"
-                                   if decompose else f"replicas x{world}"),
+                                   f"half-spinor faces {'stored peer-to-peer into symmetric memory' if comm_kind == 'p2p' else 'over NCCL'}"
+                                   if decompose else f"replicas x{world}" + (f" (fallback: {shard_fallback})" if shard_fallback else "")),
                    "l2_policy": "inputs larger than L2 (links + vectors >= 1.4 GB fp32), no flush needed"},
         "dn_applies_per_s": (1 if decompose else world) * args.steps / (ms * 1e-3),
         "q_stencils_per_s": (1 if decompose else world) * args.steps * stencils / (ms * 1e-3),

@@ -3,7 +3,7 @@ torch.distributed: one process per GPU, NCCL send/recv over NVLink for the two h
 all-reduce for the reductions.  Plumbing only: what is sent is packed, and what is received is consumed, by the library's kernels.
 
     ctx = Context(local_dims, ...); ctx.set_gauge(U[:, t_begin:t_begin + t_local])
-    comm = TorchDistComm(ctx)            # after torch.distributed.init_process_group("nccl")
+    comm, kind = make_comm(ctx, p2p=True)   # after torch.distributed.init_process_group("nccl"); p2p falls back to NCCL
     ... every operator call on ctx now acts on the global lattice ...
 """
 import torch
@@ -51,23 +51,64 @@ class TorchDistComm:
             dist.all_reduce(t, group=self.group)
 
 
+class CommSetupError(RuntimeError):
+    """A collective set-up step failed on at least one rank; raised on EVERY rank of the group (see run_agreed)."""
+
+
+def run_agreed(stage, what, device, group=None):
+    """Run `stage()` on every rank and make the outcome unanimous: the ranks exchange a success flag (all_reduce MIN) after
+    the stage, so either all return its value or all raise CommSetupError - no rank walks into the next collective alone
+    after a peer has given up, which is how a failed set-up turns into a hang."""
+    err, val = None, None
+    try:
+        val = stage()
+    except Exception as e:                                   # noqa: BLE001 - whatever went wrong is reported, then agreed on
+        err = f"{type(e).__name__}: {e}"
+    ok = torch.tensor([0 if err else 1], dtype=torch.int32, device=device)
+    dist.all_reduce(ok, op=dist.ReduceOp.MIN, group=group)
+    if int(ok.item()) == 0:
+        raise CommSetupError(f"{what}: {err or 'failed on another rank'}")
+    return val
+
+
 class PeerComm(TorchDistComm):
     """Peer-to-peer face exchange (nd_set_halo_peers): the receive windows live in a symmetric-memory allocation that every rank
     of the node maps (torch.distributed._symmetric_memory: CUDA IPC / fabric handles over NVLink), the library's pack kernel
     stores each face straight into the neighbour's window, and `wait` is the allocation's device-side barrier enqueued on the
-    context's stream - no NCCL call on the stencil's path; reductions still go through all_reduce.  One node only."""
+    context's stream - no NCCL call on the stencil's path; reductions still go through all_reduce.  One node only.
+
+    The symmetric-memory module is private to torch and has changed between releases, so its set-up runs in stages whose
+    outcome all ranks agree on (run_agreed): if any stage fails anywhere, every rank raises CommSetupError with the context
+    left unsharded, and make_comm falls back to NCCL send/recv."""
 
     def __init__(self, ctx, group=None):
-        super().__init__(ctx, group)
+        self.ctx, self.group = ctx, group
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        self.reqs = []
         if self.world > 1:
-            import torch.distributed._symmetric_memory as symm_mem
-
             g = group if group is not None else dist.group.WORLD
-            with torch.cuda.stream(ctx.stream):
-                self.window = symm_mem.empty(4 * ctx.halo_bytes(), dtype=torch.uint8, device=ctx.torch_device)
-                self.window.zero_()
-            self.handle = symm_mem.rendezvous(self.window, g)
-            ptrs = window_pointers(list(self.handle.buffer_ptrs), self.rank, self.world)
+            dev = ctx.torch_device
+
+            def allocate():
+                import torch.distributed._symmetric_memory as symm_mem
+
+                enable = getattr(symm_mem, "enable_symm_mem_for_group", None)
+                if enable is not None:                       # needed before rendezvous in some releases, a no-op / deprecated in others
+                    try:
+                        enable(g.group_name)
+                    except Exception:                        # noqa: BLE001
+                        pass
+                with torch.cuda.stream(ctx.stream):
+                    w = symm_mem.empty(4 * ctx.halo_bytes(), dtype=torch.uint8, device=dev)
+                    w.zero_()
+                return symm_mem, w
+
+            symm_mem, self.window = run_agreed(allocate, "symmetric-memory allocation", dev, group)
+            self.handle = run_agreed(lambda: symm_mem.rendezvous(self.window, g), "symmetric-memory rendezvous", dev, group)
+            ptrs = run_agreed(lambda: window_pointers([int(p) for p in self.handle.buffer_ptrs], self.rank, self.world),
+                              "peer window pointers", dev, group)
+        ctx.set_sharding(self.rank, self.world, self.start, self.wait, self.allreduce)
+        if self.world > 1:
             ctx.set_halo_peers(*ptrs)
 
     def start(self, *a):                                   # never called in peer-to-peer mode
@@ -76,6 +117,23 @@ class PeerComm(TorchDistComm):
     def wait(self):
         with torch.cuda.stream(self.ctx.stream):
             self.handle.barrier()
+
+
+def make_comm(ctx, p2p=False, group=None, log=None):
+    """The communicator of a sharded context: PeerComm when asked for and every rank can set it up, else TorchDistComm (NCCL
+    send/recv), with the reason of the fallback handed to `log` (default: stderr of rank 0).  Returns (comm, kind)."""
+    if p2p:
+        try:
+            return PeerComm(ctx, group), "p2p"
+        except CommSetupError as e:
+            msg = f"peer-to-peer face exchange unavailable ({e}); falling back to NCCL send/recv"
+            if log is not None:
+                log(msg)
+            elif dist.get_rank(group) == 0:
+                import sys
+
+                print(msg, file=sys.stderr)
+    return TorchDistComm(ctx, group), "nccl"
 
 
 def window_pointers(all_windows, rank, world):

@@ -34,6 +34,13 @@ def main():
     err = np.linalg.norm((got - ref[tb:tb + tl]).ravel()) / np.linalg.norm(ref.ravel())
     assert err <= 1e-12, err
     assert abs(ctx.norm2(x) - np.vdot(psi.ravel(), psi.ravel()).real) <= 1e-9
+    # the faces as a checksum: |Q psi|^2 depends on both received faces of every rank and crosses the all-reduce; every rank must
+    # hold the same bits, and they must be the oracle's value
+    ny = ctx.norm2(y)
+    assert abs(ny - np.vdot(ref.ravel(), ref.ravel()).real) <= 1e-10 * ny
+    seen = [None] * world
+    dist.all_gather_object(seen, ny)
+    assert all(v == seen[0] for v in seen), seen
     dist.barrier()
     dist.destroy_process_group()
 

@@ -82,3 +82,45 @@ def test_face_exchange_schedule_gloo(tmp_path, world):
         assert o["recv_prev"] == [100.0 + prev] * 6        # what the previous rank sent "to next"
         assert o["recv_next"] == [200.0 + nxt] * 6         # what the next rank sent "to previous"
         assert o["total"] == world * (world + 1) / 2
+
+
+AGREE_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch, torch.distributed as dist
+from paper_1010_5636_b200.dist import CommSetupError, run_agreed
+dist.init_process_group("gloo")
+rank = dist.get_rank()
+cpu = torch.device("cpu")
+def fails_on_rank_1():
+    if rank == 1:
+        raise ValueError("no symmetric memory here")
+    return "window"
+out = dict(rank=rank)
+try:
+    run_agreed(fails_on_rank_1, "stage A", cpu)
+    out["A"] = "returned"
+except CommSetupError as e:
+    out["A"] = str(e)
+out["B"] = run_agreed(lambda: 10 + rank, "stage B", cpu)      # the group is still usable: the next stage succeeds everywhere
+dist.barrier()
+print(json.dumps(out))
+dist.destroy_process_group()
+"""
+
+
+def test_collective_setup_is_unanimous_gloo(tmp_path):
+    """dist.run_agreed (PeerComm's set-up must not leave ranks in different states): a stage that fails on one
+    rank raises CommSetupError on both, the failing rank naming its reason, and the following stage still runs."""
+    script = tmp_path / "agree.py"
+    script.write_text(AGREE_WORKER.format(root=ROOT))
+    port = _free_port()
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE, text=True))
+    outs = [json.loads(p.communicate(timeout=180)[0].strip().splitlines()[-1]) for p in procs]
+    assert all(p.returncode == 0 for p in procs)
+    assert outs[0]["A"] == "stage A: failed on another rank"
+    assert outs[1]["A"] == "stage A: ValueError: no symmetric memory here"
+    assert [o["B"] for o in outs] == [10, 11]
