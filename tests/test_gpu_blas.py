@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 
 from lattice_inputs import gaussian_spinor
-from tests.gpu_common import make_context, rel_l2, round_to
+from tests.gpu_common import assert_field_close, make_context, rel_l2, round_to
 
 pytestmark = pytest.mark.gpu
 
@@ -121,3 +121,41 @@ def test_dev_variants_chain_on_the_device(prec):
         ctx.block_axpy_dev(c, V, x)
     want = xa - sum(np.vdot(v.ravel(), xa.ravel()) * v for v in vs)
     assert rel_l2(ctx.unpack_spinor(x), want) <= (1e-13 if prec == 64 else 3e-7)
+
+
+@pytest.mark.parametrize("dims,l", [((64, 32, 32, 32), 8), ((32, 16, 16, 16), 50), ((32, 16, 16, 16), 3)])
+@pytest.mark.parametrize("prec", [64, 32])
+def test_block_ops_at_bench_sizes(prec, dims, l):
+    """Block dot / block axpy against numpy at the sizes bench.py runs them: 32^3x64 with l = 8 (the headline
+    step's projection) and 16^3x32 with l = 50 (config 4) / l = 3 - every branch of block_dot_cols_t's launch logic: ranges
+    capped by the partial-sum scratch or not, the block's vectors split over grid.y (small lattice, many vectors) or not."""
+    import paper_1010_5636_b200 as nd
+
+    ctx = nd.Context(dims, prec=prec, recon=12, bc_time=-1)          # BLAS-1 needs no gauge field
+    V = ctx.new_spinor(l)
+    vs = []
+    for k in range(l):
+        vs.append(round_to(gaussian_spinor(dims, seed=100 + k), prec))
+        ctx.pack_spinor(vs[k], out=V[k])
+    xh = round_to(gaussian_spinor(dims, seed=7), prec)
+    x = ctx.pack_spinor(xh)
+    got = ctx.block_dot(V, x)
+    ref = np.array([np.vdot(v.ravel(), xh.ravel()) for v in vs])
+    scale = np.linalg.norm(xh) * max(np.linalg.norm(v) for v in vs)
+    assert np.abs(got - ref).max() <= 1e-13 * scale            # fp64 accumulation of exactly representable products
+    # two columns at once (the D_N projection takes <u_k, eta> and <u_k, chi> in one pass): the device-side call
+    import torch
+
+    o2 = torch.zeros(2 * l, dtype=torch.float64, device=ctx.torch_device)
+    ctx.block_dot_dev(V, x, o2)
+    ctx.synchronize()
+    h = o2.cpu().numpy()
+    assert np.array_equal(h[0::2] + 1j * h[1::2], got)          # same kernel, same bits, result left on the device
+    rng = np.random.default_rng(5)
+    a = rng.standard_normal(l) + 1j * rng.standard_normal(l)
+    ctx.block_axpy(a, V, x)
+    refy = xh.copy()
+    for k in range(l):
+        refy += a[k] * vs[k]
+    assert_field_close(ctx.unpack_spinor(x), refy, 1e-14 if prec == 64 else 3e-7)
+    ctx.close()

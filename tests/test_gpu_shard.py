@@ -12,7 +12,7 @@ import pytest
 from lattice_inputs import gauge_field, gaussian_spinor
 from oracle import sign as osign
 from oracle import wilson, wilson_c
-from tests.gpu_common import TOL, rel_l2, round_to
+from tests.gpu_common import TOL, assert_field_close, rel_l2, round_to
 from tests.test_gpu_sign import M, PREF, QNORM, low_space
 
 pytestmark = pytest.mark.gpu
@@ -127,10 +127,10 @@ def test_sharded_Q_matches_oracle(dims, R, prec, recon, bc, peers):
 
     res = em.run(work)
     got = np.concatenate([r[0] for r in res], axis=0)
-    assert rel_l2(got, ref) <= TOL[prec], rel_l2(got, ref)
+    assert_field_close(got, ref, TOL[prec])
     assert np.abs(got - ref).max() <= (1e-11 if prec == 64 else 2e-4) * np.abs(ref).max()      # boundary slices included
     got_epi = np.concatenate([r[1] for r in res], axis=0)
-    assert rel_l2(got_epi, s0 * ref + s1 * v[0] + s2 * v[1]) <= TOL[prec]
+    assert_field_close(got_epi, s0 * ref + s1 * v[0] + s2 * v[1], TOL[prec])
     for r in res:                                                           # reductions are GLOBAL on every rank
         assert abs(r[2] - np.vdot(psi.ravel(), ref.ravel())) <= (1e-11 if prec == 64 else 1e-5) * np.linalg.norm(psi.ravel()) * np.linalg.norm(ref.ravel())
         assert abs(r[3] - np.vdot(psi.ravel(), psi.ravel()).real) <= 1e-12 * r[3] and r[2] == res[0][2]
@@ -165,7 +165,7 @@ def test_sharded_DN_and_eigensolver(peers):
 
     res = em.run(work)
     got = np.concatenate([r[0] for r in res], axis=0)
-    assert rel_l2(got, ref) <= 1e-11
+    assert_field_close(got, ref, 1e-11)
     # the eigen-solver on the sharded lattice: every rank holds the same Ritz values, and they are the global lattice's
     assert res[0][3] and np.array_equal(res[0][1], res[1][1])
     import paper_1010_5636_b200 as nd

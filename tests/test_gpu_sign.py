@@ -8,7 +8,7 @@ import pytest
 from lattice_inputs import gauge_field, gaussian_spinor
 from oracle import sign as osign
 from oracle import wilson, wilson_c
-from tests.gpu_common import make_context, rel_l2, round_to
+from tests.gpu_common import assert_field_close, make_context, rel_l2, round_to
 
 pytestmark = pytest.mark.gpu
 
@@ -66,7 +66,7 @@ def test_sign_small_no_modes(prec, recon, use_graph):
     assert ctx.launch_count() - l0 == 2 * n + 1 + 1        # 2n+1 stencils + the b_n = c_n eta scale-copy
     Q = lambda v: wilson.apply_Q(v, U, M, -1)
     ref = osign.sign_poly(Q, eta, c, eps, QNORM)
-    assert rel_l2(ctx.unpack_spinor(out), ref) <= (1e-12 if prec == 64 else 5e-6)
+    assert_field_close(ctx.unpack_spinor(out), ref, (1e-12 if prec == 64 else 5e-6), ctx=ctx)
     # replay (graph cache hit) gives the same bits
     first = ctx.unpack_spinor(out)
     ctx.apply_sign(out, x, work, use_graph=use_graph)
@@ -84,7 +84,7 @@ def test_sign_degenerate_degrees(n):
     x, out, work = ctx.pack_spinor(eta), ctx.new_spinor(), ctx.new_spinor(3)
     ctx.apply_sign(out, x, work)
     Q = lambda v: wilson.apply_Q(v, U, M, -1)
-    assert rel_l2(ctx.unpack_spinor(out), osign.sign_poly(Q, eta, c, eps, QNORM)) <= 1e-13
+    assert_field_close(ctx.unpack_spinor(out), osign.sign_poly(Q, eta, c, eps, QNORM), 1e-13, ctx=ctx)
 
 
 def test_config3_DN_8c16_fp64_l20():
@@ -107,11 +107,11 @@ def test_config3_DN_8c16_fp64_l20():
         ref = osign.apply_DN(Q, wilson.apply_gamma5, eta, c, eps, QNORM, PREF, nu, Us)
         err = np.linalg.norm((got - ref).ravel())
         assert err <= PREF * max(delta, 1e-11) * np.linalg.norm(eta.ravel())
-        assert rel_l2(got, ref) <= 1e-10                     # same c_k, V, nu
+        assert_field_close(got, ref, 1e-10)  # same c_k, V, nu
     # the projected sign itself, and sign(Q) u_k = sign(nu_k) u_k up to the non-invariance of V
     ctx.apply_sign(out, x, work)
     refs = osign.sign_projected(Q, eta, c, eps, QNORM, nu, Us)
-    assert rel_l2(ctx.unpack_spinor(out), refs) <= 1e-10
+    assert_field_close(ctx.unpack_spinor(out), refs, 1e-10, ctx=ctx)
     # Ginsparg-Wilson (P9) on the CUDA path: gamma5 D + D gamma5 - (1/c) D gamma5 D = c gamma5 (1 - S^2) ~ small
     g5 = wilson.apply_gamma5
     def D(v):

@@ -7,7 +7,7 @@ from lattice_inputs import gaussian_spinor
 from oracle import sign as osign
 from oracle import solver as osolver
 from oracle import wilson, wilson_c
-from tests.gpu_common import make_context, rel_l2, round_to
+from tests.gpu_common import assert_field_close, make_context, rel_l2, round_to
 
 pytestmark = pytest.mark.gpu
 
@@ -34,7 +34,7 @@ def test_apply_DNm(prec, mq):
     out, work = ctx.new_spinor(), ctx.new_spinor(3)
     ctx.apply_DNm(out, ctx.pack_spinor(eta), RHO, mq, work, use_graph=True)
     ref = osolver.apply_DNm(DN, eta, 1.0 / RHO, mq)
-    assert rel_l2(ctx.unpack_spinor(out), ref) <= (1e-11 if prec == 64 else 1e-5)
+    assert_field_close(ctx.unpack_spinor(out), ref, (1e-11 if prec == 64 else 1e-5), ctx=ctx)
 
 
 def test_solve_fp64_matches_oracle_cg():

@@ -7,7 +7,7 @@ import pytest
 
 from lattice_inputs import gaussian_spinor
 from oracle import wilson_c
-from tests.gpu_common import TOL, make_context, rel_l2, round_to
+from tests.gpu_common import TOL, assert_field_close, make_context, rel_l2, round_to
 
 pytestmark = pytest.mark.gpu
 
@@ -29,12 +29,12 @@ def test_every_variant_matches_the_oracle(dims, bc, recon):
         ctx.set_stencil_variant(variant)
         ctx.apply_Q(y, x, -1.6)
         got = ctx.unpack_spinor(y)
-        assert rel_l2(got, ref) <= TOL[32], (variant, rel_l2(got, ref))
+        assert_field_close(got, ref, TOL[32], ctx=ctx, tag=variant)
         results[variant] = got
         out = ctx.new_spinor()
         ctx.copy(out, d[1])
         ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])   # out aliases v2, as in the Clenshaw step
-        assert rel_l2(ctx.unpack_spinor(out), ref_epi) <= TOL[32], variant
+        assert_field_close(ctx.unpack_spinor(out), ref_epi, TOL[32], ctx=ctx, tag=variant)
     # cp.async and TMA tensor-map prefetch feed the same arithmetic, and so do the two- and the four-slot kernel: bit-identical
     assert np.array_equal(results["tile"], results["tile_tma"]) and np.array_equal(results["tile"], results["tile4"])
     assert np.array_equal(results["tile"], results["auto"])       # auto = the tiled kernel
@@ -62,13 +62,13 @@ def test_fp64_tiled_kernel_matches_the_oracle(dims, bc, recon):
         assert ctx.get_stencil_variant() == ("tile" if variant == "auto" else variant)
         ctx.apply_Q(y, x, -1.6)
         got = ctx.unpack_spinor(y)
-        assert rel_l2(got, ref) <= TOL[64], (variant, rel_l2(got, ref))
+        assert_field_close(got, ref, TOL[64], ctx=ctx, tag=variant)
         results[variant] = got
         out = ctx.new_spinor()
         ctx.copy(out, d[1])
         ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])
         fused[variant] = ctx.unpack_spinor(out)
-        assert rel_l2(fused[variant], ref_epi) <= TOL[64], variant
+        assert_field_close(fused[variant], ref_epi, TOL[64], ctx=ctx, tag=variant)
     # auto in fp64: the tiled kernel for the plain stencil; for the fused-epilogue one with recon 12 only (site-per-thread with recon 8)
     assert np.array_equal(results["auto"], results["tile"]) and np.array_equal(fused["auto"], fused["tile" if recon == 12 else "site"])
     assert np.array_equal(results["tile_tma"], results["tile"]) and np.array_equal(fused["tile_tma"], fused["tile"])
@@ -93,11 +93,11 @@ def test_x3_extent_16(dims, bc, prec, recon):
     for variant in ("site", "tile", "auto"):
         ctx.set_stencil_variant(variant)
         ctx.apply_Q(y, x, -1.6)
-        assert rel_l2(ctx.unpack_spinor(y), ref) <= TOL[prec], (variant, rel_l2(ctx.unpack_spinor(y), ref))
+        assert_field_close(ctx.unpack_spinor(y), ref, TOL[prec], ctx=ctx, tag=variant)
         out = ctx.new_spinor()
         ctx.copy(out, d[1])
         ctx.apply_Q_axpbycz(out, x, -1.6, s0, s1, d[0], s2, out, s3, d[2])
-        assert rel_l2(ctx.unpack_spinor(out), ref_epi) <= TOL[prec], variant
+        assert_field_close(ctx.unpack_spinor(out), ref_epi, TOL[prec], ctx=ctx, tag=variant)
     import paper_1010_5636_b200 as nd
     for variant in ("tile4", "tile_tma"):                            # the four-slot and tensor-map kernels: x3 extent 32 only
         with pytest.raises(nd.NDError):

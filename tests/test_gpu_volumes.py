@@ -6,7 +6,7 @@ import pytest
 from lattice_inputs import gaussian_spinor
 from oracle import sign as osign
 from oracle import wilson, wilson_c
-from tests.gpu_common import TOL, make_context, rel_l2, round_to
+from tests.gpu_common import TOL, assert_field_close, make_context, rel_l2, round_to
 
 pytestmark = pytest.mark.gpu
 
@@ -19,7 +19,7 @@ def test_Q_on_24_cubed(prec, recon, dims):
     psi = round_to(gaussian_spinor(dims), prec)
     y = ctx.new_spinor()
     ctx.apply_Q(y, ctx.pack_spinor(psi), -1.6)
-    assert rel_l2(ctx.unpack_spinor(y), wilson_c.apply_Q(psi, U, -1.6, -1)) <= TOL[prec]
+    assert_field_close(ctx.unpack_spinor(y), wilson_c.apply_Q(psi, U, -1.6, -1), TOL[prec], ctx=ctx)
 
 
 def test_DN_on_24_cubed():
@@ -33,4 +33,4 @@ def test_DN_on_24_cubed():
     ctx.apply_DN(out, ctx.pack_spinor(eta), pref, work, use_graph=True)
     Q = wilson_c.make_Q(U, -1.6, -1)
     ref = osign.apply_DN(Q, wilson.apply_gamma5, eta, c, eps, qnorm, pref)
-    assert rel_l2(ctx.unpack_spinor(out), ref) <= 1e-11
+    assert_field_close(ctx.unpack_spinor(out), ref, 1e-11, ctx=ctx)

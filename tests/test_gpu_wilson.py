@@ -5,7 +5,7 @@ import pytest
 
 from lattice_inputs import gauge_field, gaussian_spinor
 from oracle import su3, wilson, wilson_c
-from tests.gpu_common import TOL, make_context, rel_l2, round_to
+from tests.gpu_common import TOL, assert_field_close, make_context, rel_l2, round_to
 
 pytestmark = pytest.mark.gpu
 
@@ -23,7 +23,7 @@ def test_config0_4x4_haar(prec, recon, bc):
     ctx.apply_Q(y, x, 0.1)
     got = ctx.unpack_spinor(y)
     ref = wilson.apply_Q(psi, U, 0.1, bc)
-    assert rel_l2(got, ref) <= TOL[prec]
+    assert_field_close(got, ref, TOL[prec], ctx=ctx)
 
 
 @pytest.mark.parametrize("recon", [18, 12])
@@ -48,7 +48,7 @@ def test_config0_free_field_plane_wave(prec, recon):
     x = ctx.pack_spinor(psi)
     y = ctx.new_spinor()
     ctx.apply_Q(y, x, m)
-    assert rel_l2(ctx.unpack_spinor(y), ref) <= (1e-12 if prec == 64 else 2e-6)
+    assert_field_close(ctx.unpack_spinor(y), ref, (1e-12 if prec == 64 else 2e-6), ctx=ctx)
 
 
 def test_recon8_flags_unit_links():
@@ -112,7 +112,7 @@ def test_ragged_lattices(prec, recon, dims):
     y = ctx.new_spinor()
     ctx.apply_Q(y, ctx.pack_spinor(psi), -1.6)
     ref = wilson_c.apply_Q(psi, U, -1.6, -1)
-    assert rel_l2(ctx.unpack_spinor(y), ref) <= TOL[prec]
+    assert_field_close(ctx.unpack_spinor(y), ref, TOL[prec], ctx=ctx)
 
 
 @pytest.mark.parametrize("recon", [12, 8])
@@ -126,12 +126,12 @@ def test_config1_16c32(prec, recon):
     y = ctx.new_spinor()
     ctx.apply_Q(y, x, -1.6)
     ref = wilson_c.apply_Q(psi, U, -1.6, -1)
-    assert rel_l2(ctx.unpack_spinor(y), ref) <= TOL[prec]
+    assert_field_close(ctx.unpack_spinor(y), ref, TOL[prec], ctx=ctx)
     # Q^2 through the temporary
     z, t = ctx.new_spinor(), ctx.new_spinor()
     ctx.apply_Q2(z, x, t, -1.6)
     ref2 = wilson_c.apply_Q(ref, U, -1.6, -1)
-    assert rel_l2(ctx.unpack_spinor(z), ref2) <= 2 * TOL[prec]
+    assert_field_close(ctx.unpack_spinor(z), ref2, 2 * TOL[prec], ctx=ctx)
 
 
 @pytest.mark.parametrize("prec", [64, 32])
@@ -144,11 +144,11 @@ def test_fused_epilogue(prec):
     s0, s1, s2, s3 = 0.37, -1.2, -1.0, 0.81
     ctx.apply_Q_axpbycz(d[2], d[0], -1.6, s0, s1, d[1], s2, d[2], s3, d[3])
     ref = s0 * wilson.apply_Q(f[0], U, -1.6, -1) + s1 * f[1] + s2 * f[2] + s3 * f[3]
-    assert rel_l2(ctx.unpack_spinor(d[2]), ref) <= TOL[prec]
+    assert_field_close(ctx.unpack_spinor(d[2]), ref, TOL[prec], ctx=ctx)
     # null vectors with zero scalars
     out = ctx.new_spinor()
     ctx.apply_Q_axpbycz(out, d[0], -1.6, 2.0)
-    assert rel_l2(ctx.unpack_spinor(out), 2.0 * wilson.apply_Q(f[0], U, -1.6, -1)) <= TOL[prec]
+    assert_field_close(ctx.unpack_spinor(out), 2.0 * wilson.apply_Q(f[0], U, -1.6, -1), TOL[prec], ctx=ctx)
 
 
 def test_aliasing_is_rejected():
