@@ -9,7 +9,8 @@
 //
 // Every Clenshaw step is two stencil launches; the vector update is the epilogue of the second one
 // (nd_apply_Q_axpbycz), so the recurrence vectors are read/written exactly once per step: 2n+1 stencil launches per
-// sign application, no separate axpy kernels.  No host synchronisation anywhere: the projection coefficients stay on
+// sign application and nothing else - no axpy kernels, and no copy for b_n = c_n eta either (its factor rides in the scalars of
+// the first two steps).  No host synchronisation anywhere: the projection coefficients stay on
 // the device, so the whole application can be replayed as one CUDA graph.
 #include <algorithm>
 #include <cmath>
@@ -17,17 +18,6 @@
 #include "nd_internal.cuh"
 
 namespace {
-
-template <typename T>
-__global__ void scale_copy_kernel(typename Prec<T>::Vec* __restrict__ y, const typename Prec<T>::Vec* __restrict__ x, T a, long long nwords) {
-    for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < nwords; w += (long long)gridDim.x * blockDim.x) {
-        typename Prec<T>::Vec v = x[w];
-        T* pv = reinterpret_cast<T*>(&v);
-#pragma unroll
-        for (int k = 0; k < (int)(sizeof(v) / sizeof(T)); k++) pv[k] *= a;
-        y[w] = v;
-    }
-}
 
 // coef_jk = sign(nu_k) <u_k,eta_j> - <u_k,chi_j> for nb right-hand sides
 // (dots = [<u,eta_0> (2l) | ... | <u,eta_{nb-1}> | <u,chi_0> (2l) | ... | <u,chi_{nb-1}>], coef[(j*l + k)*2])
@@ -38,15 +28,6 @@ __global__ void lowmode_coef_kernel(double* __restrict__ coef, const double* __r
     const double sg = (nu[k] > 0.0) ? 1.0 : ((nu[k] < 0.0) ? -1.0 : 0.0);
     coef[2 * i] = sg * dots[2 * i] - dots[2 * (l * nb + i)];
     coef[2 * i + 1] = sg * dots[2 * i + 1] - dots[2 * (l * nb + i) + 1];
-}
-
-int scale_copy(nd_ctx* ctx, void* y, const void* x, double a, int nb) {
-    const long long nwords = (long long)nb * ctx->V * (ctx->prec == 32 ? 6 : 12);
-    long long b = (nwords + 255) / 256;
-    if (ctx->prec == 32) scale_copy_kernel<float><<<(unsigned)b, 256, 0, ctx->stream>>>((float4*)y, (const float4*)x, (float)a, nwords);
-    else scale_copy_kernel<double><<<(unsigned)b, 256, 0, ctx->stream>>>((double2*)y, (const double2*)x, a, nwords);
-    ND_LAUNCHED(ctx);
-    return ND_OK;
 }
 
 // kind 0: out = sign(Q) in ; kind 1: out = pa in + pb gamma5 sign(Q) in ; for nb right-hand sides stored back to back
@@ -66,15 +47,19 @@ int enqueue_sign(nd_ctx* ctx, int nb, void* out, const void* eta, void* work, in
         rc = ndi_apply_Q_batch(ctx, nb, out, eta, m, true, c[0] / ctx->qnorm, 0, nullptr, 0, nullptr, 0, nullptr);
         if (rc != ND_OK) return rc;
     } else {
-        rc = scale_copy(ctx, bA, eta, c[n], nb);   // b_n = c_n eta ; b_{n+1} = 0 is never materialised
-        if (rc != ND_OK) return rc;
+        // b_n = c_n eta is never materialised (nor b_{n+1} = 0): the first step reads eta itself and carries c_n in its scalars,
+        //   b_{n-1} = f alpha c_n Q Q eta + (f beta c_n + c_{n-1}) eta,
+        // and the second step's "- b_n" becomes part of its eta term, (c_{n-2} - c_n) eta.  2n + 1 launches, no copy kernel.
         for (int k = n - 1; k >= 0; k--) {
             // tmp = Q b_{k+1};   b_k = f*(alpha Q tmp + beta b_{k+1}) - b_{k+2} + c_k eta,  f = 2 (k >= 1) or 1 (k = 0)
-            rc = ndi_apply_Q_batch(ctx, nb, tmp, bA, m, false, 1, 0, nullptr, 0, nullptr, 0, nullptr);
+            const bool first = (k == n - 1), second = (k == n - 2);
+            rc = ndi_apply_Q_batch(ctx, nb, tmp, first ? eta : bA, m, false, 1, 0, nullptr, 0, nullptr, 0, nullptr);
             if (rc != ND_OK) return rc;
             const double f = (k >= 1) ? 2.0 : 1.0;
-            const double s2 = (k == n - 1) ? 0.0 : -1.0;
-            rc = ndi_apply_Q_batch(ctx, nb, bB, tmp, m, true, f * alpha, f * beta, bA, s2, bB, c[k], eta);
+            if (first)
+                rc = ndi_apply_Q_batch(ctx, nb, bB, tmp, m, true, f * alpha * c[n], 0, nullptr, 0, nullptr, f * beta * c[n] + c[k], eta);
+            else
+                rc = ndi_apply_Q_batch(ctx, nb, bB, tmp, m, true, f * alpha, f * beta, bA, second ? 0.0 : -1.0, bB, second ? c[k] - c[n] : c[k], eta);
             if (rc != ND_OK) return rc;
             char* t = bA; bA = bB; bB = t;
         }
