@@ -481,6 +481,21 @@ int choose_segments(int L0, int ntile, int slots) {
     return best;
 }
 
+// fp64 plain stencil, one right-hand side, x3 extent 32: the count measured to be fastest (round-3 rows; 32^3 x 32 / 64 /
+// 128 and 96 x 16 x 32^2, every candidate timed from a cooled board).  The round model above is right for fp32 but not here, where
+// two CTAs per SM leave the kernel latency-bound and a partly filled last round costs little: the FEWEST segments that still give
+// about 3.5 rounds of CTAs win (1024 CTAs on 296 slots in all four lattices: 32^3x64 4 segments 284.9 us against 289.0 for the
+// model's 8; 32^3x32 147.1 / 151.9; 96x16x32^2 218.6 / 226.4; 32^3x128 564.3 / 565.3) - the prologue (previous slice's spinor and
+// link, read without overlap) is dear in fp64.  Only ever fewer segments than the model, the direction that was measured.
+// (The fused-epilogue launch prefers segments of 4 slices from a cooled board, 472.9 against 483.0 us, but loses that and more
+// inside a sustained loop at the power cap - 505.6 against 492.8 us - so it stays on the model.)
+int choose_segments_fp64_plain(int L0, int ntile, int slots, int model) {
+    int nseg = (int)((3.4 * slots + ntile - 1) / ntile);
+    if (nseg > model) nseg = model;
+    if (nseg > L0 / 3) nseg = L0 / 3;
+    return nseg < 1 ? 1 : nseg;
+}
+
 // ------------------------------------------------------------------------------------------ the fp64 variant
 // In fp64 a site's state is twice as large, and the kernel above neither fits the register file (next spinor of the column
 // and a whole kept link on top of accumulators, current spinor and carried time hop: 255 registers and spills) nor shared
@@ -723,7 +738,8 @@ int launch_tile2(nd_ctx* ctx, int nrhs, void* out, const void* in, double m, dou
         if (n < 1) return nd_fail(ctx, ND_ERR_CUDA, "tiled fp64 stencil does not fit on an SM");
         per_sm = n;
     }
-    const int nseg = choose_segments(G.L0, G.ntile * nrhs, per_sm * ctx->num_sms);   // a batch = more columns to march along
+    int nseg = choose_segments(G.L0, G.ntile * nrhs, per_sm * ctx->num_sms);   // a batch = more columns to march along
+    if (sizeof(T) == 8 && !EPI && nrhs == 1 && L3 == 32) nseg = choose_segments_fp64_plain(G.L0, G.ntile, per_sm * ctx->num_sms, nseg);
     G.seg_base = G.L0 / nseg;
     G.seg_rem = G.L0 % nseg;
     const dim3 blocks((unsigned)(G.ntile * nseg), (unsigned)nrhs, 1);
